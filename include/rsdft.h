@@ -1,0 +1,147 @@
+/*
+ * rsdft.h -- C ABI of librsdft: the data-parallel hot path of one LOBPCG block step of
+ * real-space Kohn-Sham DFT (arXiv 2512.04447 "QUMASUN": (1) FFT Laplacian,
+ * (2) H and S matrices of LOBPCG, (4) nonlocal pseudopotential operator), B200 / sm_100a.
+ *
+ * Notation: grid N = (Nx, Ny, Nz), Ng = Nx*Ny*Nz, periodic
+ * orthorhombic box L (bohr), h_a = L_a / N_a, dV = hx*hy*hz; grid point (ix, iy, iz) sits at
+ * r = (ix*hx, iy*hy, iz*hz) and has linear index g = (ix*Ny + iy)*Nz + iz (z fastest).
+ * An orbital block is `ncol` columns; column c starts at element c*ld (ld >= Ng); every
+ * element is complex128, interleaved (re, im) = 16 bytes.  Hartree atomic units.
+ *
+ * All entry points return 0 (RSDFT_OK) or a negative rsdft_status; they never throw or
+ * abort.  On error the outputs are undefined and rsdft_last_error() (thread-local) carries
+ * a message.  "device" pointers are CUDA device pointers of the current device; "host"
+ * pointers are ordinary host memory.  `stream` is a cudaStream_t passed as void* (NULL =
+ * the legacy default stream).  The compute calls are asynchronous on `stream` and never
+ * synchronise with the host; a plan owns one workspace, so at most one call per plan may
+ * be in flight at a time (calls on the same stream are naturally ordered).
+ */
+#ifndef RSDFT_H
+#define RSDFT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    RSDFT_OK = 0,
+    RSDFT_INVALID_ARG = -1, /* null pointer, ncol <= 0, ld < Ng, X aliases HX, |m| > l, l > 2, ... */
+    RSDFT_UNSUPPORTED = -2, /* grid length outside {16,32,48,64,80,96,112,128}; box <= 0; 2*rc >= min L */
+    RSDFT_ALLOC = -3,       /* host or device allocation failed */
+    RSDFT_CUDA = -4         /* CUDA runtime error; message carries cudaGetErrorString */
+} rsdft_status;
+
+typedef struct rsdft_plan rsdft_plan_t; /* opaque, library-owned */
+
+typedef struct { int32_t n[3]; } rsdft_grid_t;   /* Nx, Ny, Nz */
+typedef struct { double len[3]; } rsdft_box_t;   /* Lx, Ly, Lz in bohr */
+
+typedef struct {
+    int32_t natom;          /* may be 0 */
+    const double *pos;      /* host [natom][3], bohr, absolute; wrapped into [0, L) by the plan */
+    const int32_t *species; /* host [natom], index into rsdft_projectors_t.species */
+} rsdft_atoms_t;
+
+/* One species' Kleinman-Bylander projectors  beta_i(r) = f_i(|d|) * Y_{l_i m_i}(d/|d|),
+ * d = minimum-image displacement from the atom, truncated to the sphere |d|^2 < rc^2
+ * (strict; |d|^2 = dx*dx + dy*dy + dz*dz in double).  Y_lm are the real spherical
+ * harmonics, orthonormal on the unit sphere:  Y00 = 1/(2 sqrt(pi));
+ * l=1: sqrt(3/4pi) * {y, z, x}/r for m = -1, 0, 1;
+ * l=2: 1/2 sqrt(15/pi) xy/r^2, 1/2 sqrt(15/pi) yz/r^2, 1/4 sqrt(5/pi) (3z^2 - r^2)/r^2,
+ *      1/2 sqrt(15/pi) xz/r^2, 1/4 sqrt(15/pi) (x^2 - y^2)/r^2 for m = -2..2.
+ * At |d| = 0: Y00 as usual, 0 for l > 0.   (BASELINE.json configs[0]; R7-R9.) */
+typedef struct {
+    double rc;              /* bohr, > 0, 2*rc < min L */
+    int32_t nproj;          /* 1..16 */
+    const int32_t *l;       /* host [nproj], 0..2 */
+    const int32_t *m;       /* host [nproj], -l..l */
+    int32_t radial_kind;    /* 0: f_i(r) = exp(-alpha[i] r^2);  1: table, linear interpolation */
+    const double *alpha;    /* host [nproj]            (kind 0) */
+    int32_t nr;             /* table length >= 2       (kind 1) */
+    double dr;              /* table spacing, bohr     (kind 1): sample j is f(j*dr); f = 0 for r >= (nr-1)*dr */
+    const double *radial;   /* host [nproj][nr]        (kind 1) */
+    const double *D;        /* host [nproj][nproj], real symmetric coupling, Hartree */
+} rsdft_species_t;
+
+typedef struct {
+    int32_t nspecies;
+    const rsdft_species_t *species; /* host [nspecies] */
+} rsdft_projectors_t;
+
+/* Build a plan for a grid, a box, atoms and their projectors (BASELINE.json north_star:
+ * "rsdft_plan_create(grid, box, atoms, projectors)").  Everything passed in is host memory
+ * and is copied; the caller may free it on return.  The plan precomputes, once:
+ *   - the kinetic factors t(k) = 1/2 sum_a (2 pi kappa_a / L_a)^2, kappa = k for k < N/2 else
+ *     k - N (configs[0]), stored separably with 1/Ng folded in, and the FFT twiddles;
+ *   - per atom: the list of grid points inside its sphere (int32 g), the table
+ *     beta[nproj][npts] (double) and D.
+ * atoms == NULL / natom == 0 / projectors == NULL gives H = T + V_loc.  V_loc is 0 until
+ * rsdft_plan_set_vloc is called.  *out receives the plan.  Must be called with the target
+ * CUDA device current; the plan is bound to that device.
+ * Errors: INVALID_ARG, UNSUPPORTED, ALLOC, CUDA. */
+int rsdft_plan_create(const rsdft_grid_t *grid, const rsdft_box_t *box, const rsdft_atoms_t *atoms,
+                      const rsdft_projectors_t *projectors, rsdft_plan_t **out);
+
+/* Set the local potential v(r): vloc_dev is a DEVICE array [Ng] of doubles; it is copied
+ * into a plan-owned buffer asynchronously on `stream` (the caller's array is not retained).
+ * PAPER.md:79 ("density and potential updates" happen every SCF iteration while grid,
+ * atoms and projectors stay fixed).  NULL resets V_loc to 0. */
+int rsdft_plan_set_vloc(rsdft_plan_t *plan, const double *vloc_dev, void *stream);
+
+/* HX = (-1/2 Laplacian + V_loc + V_NL) X  for ncol columns (PAPER.md:19 tasks (1), (4);
+ * north_star "rsdft_apply_h(X -> HX)"):
+ *   T:    psi^(k) = sum_r psi(r) e^{-2 pi i sum_a k_a i_a / N_a};  psi^ *= t(k);
+ *         (T psi)(r) = 1/Ng sum_k psi^(k) e^{+2 pi i ...}
+ *   Vloc: + v(r) psi(r)
+ *   VNL:  for every atom a: p_i = dV sum_{r in S_a} beta_i(r) psi(r);
+ *         HX(r) += sum_ij beta_i(r) D_ij p_j for r in S_a.
+ * X, HX: DEVICE, complex128, column c at element offset c*ldx / c*ldhx, ldx, ldhx >= Ng.
+ * X is read-only; HX must not overlap X (HX doubles as FFT scratch).  Any ncol >= 1.
+ * Errors: INVALID_ARG, CUDA. */
+int rsdft_apply_h(rsdft_plan_t *plan, int32_t ncol, const void *X, int64_t ldx,
+                  void *HX, int64_t ldhx, void *stream);
+
+/* Rayleigh-Ritz Gram matrices of LOBPCG (PAPER.md:19 task (2); north_star
+ * "rsdft_subspace_gram(Y, HY -> H_sub, S_sub)") for Y = [X, W, P] with n columns:
+ *   S_sub[i,j] = sum_r conj(Y[r,i]) Y[r,j],   H_sub[i,j] = sum_r conj(Y[r,i]) HY[r,j]
+ * (plain sums, no dV).  Y, HY: DEVICE complex128, column c at c*ldy / c*ldhy.
+ * H_sub, S_sub: DEVICE, n x n complex128, column-major, element (i,j) at i + j*lds,
+ * lds >= n; both triangles are written.  S_sub is exactly Hermitian; H_sub is computed in
+ * full (Hermitian only to round-off).  Either of H_sub (with HY) or S_sub may be NULL to
+ * skip it.  Errors: INVALID_ARG, ALLOC, CUDA. */
+int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ldy,
+                        const void *HY, int64_t ldhy, void *H_sub, void *S_sub, int32_t lds,
+                        void *stream);
+
+/* One whole block step with HOST buffers (the end-to-end entry point): copies Y
+ * (host, pinned recommended) to the device in column chunks overlapped with rsdft_apply_h,
+ * forms HY = H Y on the device, then the Gram matrices, and copies H_sub, S_sub (and HY if
+ * HY_host != NULL) back to the host.  Synchronises with the host before returning.
+ * Y_host/HY_host: HOST complex128 [n][ld]; H_sub_host, S_sub_host: HOST n x n column-major.
+ * Errors: INVALID_ARG, ALLOC, CUDA. */
+int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int64_t ldy,
+                          void *HY_host, int64_t ldhy, void *H_sub_host, void *S_sub_host,
+                          int32_t lds);
+
+/* Introspection used by tests/bench: fills out[0..7] with
+ *   {natom, total sphere points, max points per sphere, device bytes owned by the plan,
+ *    apply_h column batch width, kernels launched by the last compute call, Ng, reserved}. */
+int rsdft_plan_info(const rsdft_plan_t *plan, int64_t *out8);
+
+/* Tuning knob: number of columns apply_h pushes through its kernel sequence at a time
+ * (0 = library default, chosen so one batch stays L2-resident). */
+int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols);
+
+/* Destroys the plan and frees everything it owns (synchronises the device first). */
+int rsdft_plan_destroy(rsdft_plan_t *plan);
+
+/* Thread-local message of the last failing call on this thread ("" if none). */
+const char *rsdft_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RSDFT_H */

@@ -1,0 +1,203 @@
+// Rayleigh-Ritz Gram matrices of LOBPCG (PAPER.md:19 task (2) "GEMM to construct the Hamiltonian
+// and overlap matrices"):
+//   S_sub[i,j] = sum_r conj(Y[r,i]) Y[r,j],    H_sub[i,j] = sum_r conj(Y[r,i]) HY[r,j].
+//
+// This is the one dense contraction of the path, so it runs on the FP64 tensor pipe: the only
+// native FP64 MMA shape on sm_100a is DMMA.8x8x4 (mma.sync.m8n8k4.f64).  Both operands are
+// "K-major" in memory (a column of Y is contiguous in r), which is exactly the row (A) / col (B)
+// fragment layout of m8n8k4, so tiles are staged into shared memory as plain interleaved
+// complex128 with cp.async and read back as one 128-bit LDS per fragment (re, im).
+//
+// One complex product = 4 real MMAs:  re += Ar*Br;  re += Ai*Bi;  im += Ar*Bi;  im += (-Ai)*Br.
+//
+// Work decomposition: a unit = (K-slab, output tile).  Tiles are TM x TN complex; S_sub only
+// needs its upper-triangular tiles (it is exactly Hermitian), H_sub is computed in full.
+// Units are ordered slab-major so the ~148 CTAs resident at any time stream the SAME grid-point
+// range and share their Y / HY panels through L2.  Every unit writes its partial tile to a
+// workspace; gram_reduce_kernel then sums the slabs in a fixed order (deterministic), mirrors
+// S_sub and writes both triangles.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rsdft {
+
+struct GramTile { int16_t ti, tj, mat, pad; };   // mat 0: H_sub = Y^H HY, 1: S_sub = Y^H Y
+
+struct GramArgs {
+    const double2 *Y, *HY;
+    int64_t ldy, ldhy;
+    int32_t n;                 // columns
+    int32_t ntiles;            // entries of `tiles`
+    int32_t kslabs;            // K split
+    int64_t nchunks;           // Ng / KC
+    const GramTile *tiles;
+    double2 *work;             // [kslabs][2][n*n] column-major partials (mat 0 = H, 1 = S)
+};
+
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+
+// CTA tile (WGM*FA*8) x (WGN*FB*8) complex outputs, WGM*WGN warps, each warp FA x FB DMMA tiles.
+// KC grid points per pipeline stage, smem row pitch KC+4 complex (pitch % 8 == 4 -> the 8 lanes
+// of an LDS.128 phase, 2 rows x 4 k, hit 8 distinct 16-byte bank groups).
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES>
+struct GramCfg {
+    static constexpr int TM = WGM * FA * 8, TN = WGN * FB * 8;
+    static constexpr int THREADS = WGM * WGN * 32;
+    static constexpr int PITCH = KC + 4;
+    static constexpr int STAGE_ELEMS = (TM + TN) * PITCH;           // double2
+    static constexpr size_t SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(double2);
+};
+
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES>
+__global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
+{
+    using Cfg = GramCfg<WGM, WGN, FA, FB, KC, STAGES>;
+    constexpr int TM = Cfg::TM, TN = Cfg::TN, PITCH = Cfg::PITCH, NT = Cfg::THREADS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2 *sm = reinterpret_cast<double2 *>(smem_raw);
+
+    const int unit = blockIdx.x;
+    const int ks = unit / a.ntiles;
+    const GramTile tl = a.tiles[unit - ks * a.ntiles];
+    const int i0 = tl.ti * TM, j0 = tl.tj * TN;
+    const double2 *Abase = a.Y;
+    const double2 *Bbase = tl.mat ? a.Y : a.HY;
+    const int64_t lda = a.ldy, ldb = tl.mat ? a.ldy : a.ldhy;
+    const int64_t c0 = a.nchunks * ks / a.kslabs, c1 = a.nchunks * (ks + 1) / a.kslabs;
+    const int nch = (int)(c1 - c0);
+    const int64_t r0 = c0 * KC;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp / WGN, wn = warp % WGN;
+    const int g = lane >> 2, t = lane & 3;
+
+    // stage loader: (TM+TN) rows x KC elements of 16 B; consecutive threads walk k first
+    auto load_stage = [&](int stage, int chunk) {
+        double2 *dst = sm + (size_t)stage * Cfg::STAGE_ELEMS;
+        const int64_t r = r0 + (int64_t)chunk * KC;
+#pragma unroll
+        for (int e = tid; e < (TM + TN) * KC; e += NT) {
+            const int row = e / KC, k = e - row * KC;
+            double2 *d = dst + row * PITCH + k;
+            if (row < TM) {
+                const int col = i0 + row;
+                if (col < a.n) cp_async16(d, Abase + (int64_t)col * lda + r + k);
+                else *d = make_double2(0.0, 0.0);
+            } else {
+                const int col = j0 + row - TM;
+                if (col < a.n) cp_async16(d, Bbase + (int64_t)col * ldb + r + k);
+                else *d = make_double2(0.0, 0.0);
+            }
+        }
+    };
+
+    double cre[FA][FB][2], cim[FA][FB][2];
+#pragma unroll
+    for (int x = 0; x < FA; ++x)
+#pragma unroll
+        for (int y = 0; y < FB; ++y) { cre[x][y][0] = cre[x][y][1] = 0.0; cim[x][y][0] = cim[x][y][1] = 0.0; }
+
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nch) load_stage(s, s);
+        cp_async_commit();
+    }
+
+    for (int ch = 0; ch < nch; ++ch) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {   // prefetch chunk ch+STAGES-1 into the stage consumed at iteration ch-1
+            const int nx = ch + STAGES - 1;
+            if (nx < nch) load_stage(nx % STAGES, nx);
+            cp_async_commit();
+        }
+        const double2 *As = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + (wm * FA * 8 + g) * PITCH + t;
+        const double2 *Bs = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + (TM + wn * FB * 8 + g) * PITCH + t;
+#pragma unroll
+        for (int kk = 0; kk < KC; kk += 4) {
+            double br[FB], bi[FB];
+#pragma unroll
+            for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PITCH + kk]; br[y] = v.x; bi[y] = v.y; }
+#pragma unroll
+            for (int x = 0; x < FA; ++x) {
+                const double2 v = As[x * 8 * PITCH + kk];
+                const double ar = v.x, ai = v.y, nai = -v.y;
+#pragma unroll
+                for (int y = 0; y < FB; ++y) {
+                    dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
+                    dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
+                }
+#pragma unroll
+                for (int y = 0; y < FB; ++y) {
+                    dmma884(cre[x][y][0], cre[x][y][1], ai, bi[y]);
+                    dmma884(cim[x][y][0], cim[x][y][1], nai, br[y]);
+                }
+            }
+        }
+    }
+    cp_async_wait<0>();
+
+    // epilogue: C fragment element e of (x, y) is row g, column 2t+e of that 8x8 tile
+    double2 *W = a.work + ((int64_t)ks * 2 + tl.mat) * (int64_t)a.n * a.n;
+#pragma unroll
+    for (int x = 0; x < FA; ++x)
+#pragma unroll
+        for (int y = 0; y < FB; ++y)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int i = i0 + (wm * FA + x) * 8 + g;
+                const int j = j0 + (wn * FB + y) * 8 + 2 * t + e;
+                if (i < a.n && j < a.n) W[(int64_t)j * a.n + i] = make_double2(cre[x][y][e], cim[x][y][e]);
+            }
+}
+
+// Fixed-order sum over K-slabs; H_sub written as computed, S_sub from its upper-triangular tiles:
+// element (i,j) with tile(i) < tile(j) is computed, its mirror is the conjugate; inside a diagonal
+// tile the i<j half is used and mirrored, and the diagonal's imaginary part is exactly 0
+// (S_ii = |y_i|^2), so S_sub is exactly Hermitian.
+struct GramReduceArgs {
+    const double2 *work;
+    double2 *H, *S;
+    int32_t n, lds, kslabs;
+};
+
+__global__ void __launch_bounds__(256) gram_reduce_kernel(GramReduceArgs a)
+{
+    const int64_t nn = (int64_t)a.n * a.n;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += (int64_t)gridDim.x * blockDim.x) {
+        const int j = (int)(e / a.n), i = (int)(e - (int64_t)j * a.n);
+        if (a.H) {
+            double sr = 0.0, si = 0.0;
+            for (int k = 0; k < a.kslabs; ++k) {
+                const double2 v = a.work[((int64_t)k * 2 + 0) * nn + e];
+                sr += v.x; si += v.y;
+            }
+            a.H[(int64_t)j * a.lds + i] = make_double2(sr, si);
+        }
+        if (a.S && i <= j) {
+            double sr = 0.0, si = 0.0;
+            for (int k = 0; k < a.kslabs; ++k) {
+                const double2 v = a.work[((int64_t)k * 2 + 1) * nn + e];
+                sr += v.x; si += v.y;
+            }
+            if (i == j) si = 0.0;
+            a.S[(int64_t)j * a.lds + i] = make_double2(sr, si);
+            if (i != j) a.S[(int64_t)i * a.lds + j] = make_double2(sr, -si);
+        }
+    }
+}
+
+}  // namespace rsdft

@@ -1,0 +1,705 @@
+// librsdft: host plan + C ABI (include/rsdft.h) over the sm_100a kernels in this directory.
+// PAPER.md:19 (tasks (1) FFT Laplacian, (2) H/S matrices, (4) nonlocal operator); the problem
+// statement is BASELINE.json north_star/configs; readings R1..R18 are listed in DESIGN.md.
+// Nothing here is shared with oracle/ (the CPU oracle is test infrastructure).
+#include "../../include/rsdft.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "fft_kernels.cuh"
+#include "gram_kernels.cuh"
+#include "nonlocal_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg)
+{
+    g_err = msg;
+    return code;
+}
+
+#define RS_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? RSDFT_ALLOC : RSDFT_CUDA,                \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                       \
+    } while (0)
+
+const long double PI_L = 3.14159265358979323846264338327950288L;
+
+template <class T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t n = 0;
+    ~DevBuf() { release(); }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        n = 0;
+    }
+    cudaError_t alloc(size_t count)
+    {
+        release();
+        if (count == 0) return cudaSuccess;
+        cudaError_t e = cudaMalloc((void **)&p, count * sizeof(T));
+        if (e == cudaSuccess) n = count;
+        return e;
+    }
+    cudaError_t ensure(size_t count) { return count <= n ? cudaSuccess : alloc(count); }
+    cudaError_t upload(const std::vector<T> &h)
+    {
+        cudaError_t e = alloc(h.size());
+        if (e != cudaSuccess || h.empty()) return e;
+        return cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+    }
+    size_t bytes() const { return n * sizeof(T); }
+};
+
+}  // namespace
+
+struct rsdft_plan {
+    int n[3];
+    double len[3];
+    int64_t ng;
+    double dV;
+    int device = 0;
+    int num_sms = 148;
+
+    // FFT tables
+    DevBuf<double2> tw[3];        // per axis: w_N^m = (cos, -sin)(2 pi m / N)
+    DevBuf<double> kin_x;         // t_x[kx] / Ng                       [Nx]
+    DevBuf<double> kin_yz;        // (t_y[ky] + t_z[kz]) / Ng           [Ny*Nz]
+    DevBuf<double> vloc;          // [Ng], zero until set
+
+    // projector tables
+    int natom = 0, maxproj = 0;
+    int64_t total_pts = 0, max_pts = 0;
+    DevBuf<int64_t> pt_off, beta_off;
+    DevBuf<int32_t> idx, nproj_a;
+    DevBuf<double> beta, Dmat;
+    std::vector<std::vector<int32_t>> colour_atoms;   // host copy of the colour classes
+    DevBuf<int32_t> alist;                            // concatenated colour classes
+    std::vector<int> colour_off;
+    DevBuf<double2> pq;                               // [natom][maxproj][batch]
+
+    // apply_h batching
+    int batch = 0;                // columns per kernel sequence
+    int user_batch = 0;
+
+    // gram workspace
+    DevBuf<double2> gram_work;
+    DevBuf<rsdft::GramTile> gram_tiles;
+    int gram_tiles_n = -1, gram_ntiles = 0;
+
+    // host-buffer entry point
+    DevBuf<double2> hostY, hostHY, hostHS;
+    cudaStream_t s_copy = nullptr, s_comp = nullptr;
+    std::vector<cudaEvent_t> ev;
+
+    int64_t last_launches = 0;
+
+    ~rsdft_plan()
+    {
+        for (auto e : ev) cudaEventDestroy(e);
+        if (s_copy) cudaStreamDestroy(s_copy);
+        if (s_comp) cudaStreamDestroy(s_comp);
+    }
+    size_t device_bytes() const
+    {
+        size_t b = 0;
+        for (int a = 0; a < 3; ++a) b += tw[a].bytes();
+        b += kin_x.bytes() + kin_yz.bytes() + vloc.bytes() + pt_off.bytes() + beta_off.bytes() + idx.bytes() +
+             nproj_a.bytes() + beta.bytes() + Dmat.bytes() + alist.bytes() + pq.bytes() + gram_work.bytes() +
+             gram_tiles.bytes() + hostY.bytes() + hostHY.bytes() + hostHS.bytes();
+        return b;
+    }
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------
+// host-side table construction (long double, rounded once)
+
+// kappa(j) = j for j < N/2 else j - N  (BASELINE.json configs[0]; R2)
+inline long kappa_of(long j, long n) { return 2 * j < n ? j : j - n; }
+
+// real spherical harmonics, orthonormal on the unit sphere (R7, R8)
+long double real_ylm(int l, int m, long double x, long double y, long double z)
+{
+    if (l == 0) return 0.5L / sqrtl(PI_L);
+    const long double r2 = x * x + y * y + z * z;
+    if (r2 == 0.0L) return 0.0L;
+    if (l == 1) {
+        const long double c = sqrtl(0.75L / PI_L) / sqrtl(r2);
+        return c * (m < 0 ? y : (m == 0 ? z : x));
+    }
+    const long double a = sqrtl(15.0L / PI_L) / r2, b = sqrtl(5.0L / PI_L) / r2;
+    switch (m) {
+    case -2: return 0.5L * a * x * y;
+    case -1: return 0.5L * a * y * z;
+    case 0: return 0.25L * b * (3.0L * z * z - r2);
+    case 1: return 0.5L * a * x * z;
+    default: return 0.25L * a * (x * x - y * y);
+    }
+}
+
+long double radial_part(const rsdft_species_t &sp, int i, long double r)
+{
+    if (sp.radial_kind == 0) return expl(-(long double)sp.alpha[i] * r * r);
+    const long double u = r / (long double)sp.dr;
+    const long j = (long)floorl(u);
+    if (j >= sp.nr - 1) return 0.0L;
+    const double *tab = sp.radial + (size_t)i * sp.nr;
+    return (long double)tab[j] + (u - (long double)j) * ((long double)tab[j + 1] - (long double)tab[j]);
+}
+
+// minimum-image displacement, evaluated in double (R5, R6: membership is decided in
+// double as dx*dx + dy*dy + dz*dz < rc*rc)
+inline double min_img(double r, double R, double L)
+{
+    const double d = r - R;
+    return d - L * std::nearbyint(d / L);
+}
+
+int validate_species(const rsdft_species_t &sp, const double len[3], int s)
+{
+    const std::string tag = "species " + std::to_string(s) + ": ";
+    if (!(sp.rc > 0.0)) return fail(RSDFT_INVALID_ARG, tag + "rc must be > 0");
+    if (sp.nproj < 1 || sp.nproj > 16) return fail(RSDFT_INVALID_ARG, tag + "nproj must be in 1..16");
+    if (!sp.l || !sp.m || !sp.D) return fail(RSDFT_INVALID_ARG, tag + "null l/m/D");
+    for (int i = 0; i < sp.nproj; ++i) {
+        if (sp.l[i] < 0 || sp.l[i] > 2) return fail(RSDFT_INVALID_ARG, tag + "l must be 0..2");
+        if (std::abs(sp.m[i]) > sp.l[i]) return fail(RSDFT_INVALID_ARG, tag + "|m| > l");
+    }
+    if (sp.radial_kind == 0) {
+        if (!sp.alpha) return fail(RSDFT_INVALID_ARG, tag + "null alpha");
+    } else if (sp.radial_kind == 1) {
+        if (!sp.radial || sp.nr < 2 || !(sp.dr > 0.0)) return fail(RSDFT_INVALID_ARG, tag + "bad radial table");
+    } else {
+        return fail(RSDFT_INVALID_ARG, tag + "radial_kind must be 0 or 1");
+    }
+    for (int i = 0; i < sp.nproj; ++i)
+        for (int j = 0; j < i; ++j)
+            if (sp.D[i * sp.nproj + j] != sp.D[j * sp.nproj + i]) return fail(RSDFT_INVALID_ARG, tag + "D not symmetric");
+    const double lmin = std::min(len[0], std::min(len[1], len[2]));
+    if (!(2.0 * sp.rc < lmin)) return fail(RSDFT_UNSUPPORTED, tag + "2*rc >= min box length (one periodic image only)");
+    return RSDFT_OK;
+}
+
+int build_spheres(rsdft_plan *P, const rsdft_atoms_t *atoms, const rsdft_projectors_t *proj)
+{
+    const int natom = atoms->natom;
+    P->natom = natom;
+    int maxproj = 0;
+    for (int a = 0; a < natom; ++a) {
+        const int s = atoms->species[a];
+        if (s < 0 || s >= proj->nspecies) return fail(RSDFT_INVALID_ARG, "atom species index out of range");
+        maxproj = std::max(maxproj, proj->species[s].nproj);
+    }
+    P->maxproj = maxproj;
+    const double h[3] = {P->len[0] / P->n[0], P->len[1] / P->n[1], P->len[2] / P->n[2]};
+
+    std::vector<int64_t> pt_off(natom + 1, 0), beta_off(natom, 0);
+    std::vector<int32_t> idx, nproj_a(natom);
+    std::vector<double> beta, Dm((size_t)natom * maxproj * maxproj, 0.0);
+    int64_t max_pts = 0;
+    for (int a = 0; a < natom; ++a) {
+        const rsdft_species_t &sp = proj->species[atoms->species[a]];
+        const double *R = atoms->pos + 3 * a;
+        const double rc2 = sp.rc * sp.rc;
+        // per-axis candidates: |d_axis|^2 < rc^2 is necessary for membership
+        std::vector<int> cand[3];
+        std::vector<double> dc[3];
+        for (int ax = 0; ax < 3; ++ax)
+            for (int i = 0; i < P->n[ax]; ++i) {
+                const double d = min_img(i * h[ax], R[ax], P->len[ax]);
+                if (d * d < rc2) { cand[ax].push_back(i); dc[ax].push_back(d); }
+            }
+        std::vector<int32_t> my;
+        std::vector<double> mx, myy, mz;
+        for (size_t ix = 0; ix < cand[0].size(); ++ix)
+            for (size_t iy = 0; iy < cand[1].size(); ++iy)
+                for (size_t iz = 0; iz < cand[2].size(); ++iz) {
+                    const double dx = dc[0][ix], dy = dc[1][iy], dz = dc[2][iz];
+                    const double d2 = dx * dx + dy * dy + dz * dz;
+                    if (!(d2 < rc2)) continue;
+                    my.push_back((int32_t)(((int64_t)cand[0][ix] * P->n[1] + cand[1][iy]) * P->n[2] + cand[2][iz]));
+                    mx.push_back(dx); myy.push_back(dy); mz.push_back(dz);
+                }
+        const int64_t np = (int64_t)my.size();
+        max_pts = std::max(max_pts, np);
+        pt_off[a + 1] = pt_off[a] + np;
+        beta_off[a] = (int64_t)beta.size();
+        nproj_a[a] = sp.nproj;
+        idx.insert(idx.end(), my.begin(), my.end());
+        beta.resize(beta.size() + (size_t)np * sp.nproj);
+        double *bt = beta.data() + beta_off[a];
+        for (int64_t s = 0; s < np; ++s) {
+            const long double x = mx[s], y = myy[s], z = mz[s];
+            const long double r = sqrtl(x * x + y * y + z * z);
+            for (int i = 0; i < sp.nproj; ++i)
+                bt[(int64_t)i * np + s] = (double)(radial_part(sp, i, r) * real_ylm(sp.l[i], sp.m[i], x, y, z));
+        }
+        for (int i = 0; i < sp.nproj; ++i)
+            for (int j = 0; j < sp.nproj; ++j)
+                Dm[((size_t)a * maxproj + i) * maxproj + j] = sp.D[i * sp.nproj + j];
+    }
+    P->total_pts = pt_off[natom];
+    P->max_pts = max_pts;
+
+    // colour classes: atoms whose spheres may share a grid point (|R_a - R_b|_min-image < rc_a + rc_b)
+    // get different colours; scatter-add then runs one launch per class without atomics.
+    std::vector<int> colour(natom, -1);
+    int ncolour = 0;
+    for (int a = 0; a < natom; ++a) {
+        std::vector<char> used(ncolour + 1, 0);
+        for (int b = 0; b < a; ++b) {
+            double d2 = 0.0;
+            for (int ax = 0; ax < 3; ++ax) {
+                const double d = min_img(atoms->pos[3 * a + ax], atoms->pos[3 * b + ax], P->len[ax]);
+                d2 += d * d;
+            }
+            const double rr = proj->species[atoms->species[a]].rc + proj->species[atoms->species[b]].rc +
+                              (h[0] + h[1] + h[2]);
+            if (d2 < rr * rr) used[colour[b]] = 1;
+        }
+        int c = 0;
+        while (used[c]) ++c;
+        colour[a] = c;
+        ncolour = std::max(ncolour, c + 1);
+    }
+    P->colour_atoms.assign(ncolour, {});
+    for (int a = 0; a < natom; ++a) P->colour_atoms[colour[a]].push_back(a);
+    std::vector<int32_t> alist;
+    P->colour_off.assign(1, 0);
+    for (auto &v : P->colour_atoms) {
+        alist.insert(alist.end(), v.begin(), v.end());
+        P->colour_off.push_back((int)alist.size());
+    }
+
+    RS_CUDA(P->pt_off.upload(pt_off));
+    RS_CUDA(P->beta_off.upload(beta_off));
+    RS_CUDA(P->idx.upload(idx));
+    RS_CUDA(P->nproj_a.upload(nproj_a));
+    RS_CUDA(P->beta.upload(beta));
+    RS_CUDA(P->Dmat.upload(Dm));
+    RS_CUDA(P->alist.upload(alist));
+    return RSDFT_OK;
+}
+
+int build_fft_tables(rsdft_plan *P)
+{
+    for (int ax = 0; ax < 3; ++ax) {
+        const int N = P->n[ax];
+        std::vector<double2> w(N);
+        for (int m = 0; m < N; ++m) {
+            // exact octant symmetries are kept by reducing the angle before cosl/sinl
+            const long double ang = 2.0L * PI_L * (long double)m / (long double)N;
+            w[m] = make_double2((double)cosl(ang), (double)(-sinl(ang)));
+        }
+        RS_CUDA(P->tw[ax].upload(w));
+    }
+    const long double inv_ng = 1.0L / (long double)P->ng;
+    auto t_axis = [&](int ax, int k) -> long double {
+        const long double g = 2.0L * PI_L * (long double)kappa_of(k, P->n[ax]) / (long double)P->len[ax];
+        return 0.5L * g * g;
+    };
+    std::vector<double> kx(P->n[0]), kyz((size_t)P->n[1] * P->n[2]);
+    for (int i = 0; i < P->n[0]; ++i) kx[i] = (double)(t_axis(0, i) * inv_ng);
+    for (int j = 0; j < P->n[1]; ++j)
+        for (int k = 0; k < P->n[2]; ++k) kyz[(size_t)j * P->n[2] + k] = (double)((t_axis(1, j) + t_axis(2, k)) * inv_ng);
+    RS_CUDA(P->kin_x.upload(kx));
+    RS_CUDA(P->kin_yz.upload(kyz));
+    RS_CUDA(P->vloc.alloc((size_t)P->ng));
+    RS_CUDA(cudaMemset(P->vloc.p, 0, P->vloc.bytes()));
+    return RSDFT_OK;
+}
+
+}  // namespace
+
+namespace {
+
+// ------------------------------------------------------------------------------------------
+// kernel launchers
+
+using namespace rsdft;
+
+template <int N, int MODE>
+void launch_lines_n(const LinesArgs &a, int grid_cap, cudaStream_t st)
+{
+    constexpr int L = 8;   // 128 threads, 8 contiguous lines per CTA
+    const int64_t blocks = (a.nlines + L - 1) / L;
+    const int grid = (int)std::min<int64_t>(blocks, grid_cap);
+    fft_lines_kernel<N, L, MODE><<<grid, 16 * L, 0, st>>>(a);
+}
+
+template <int N, int MODE>
+void launch_strided_n(const StridedArgs &a, int grid_cap, cudaStream_t st)
+{
+    constexpr int T = 8;   // 128 threads, 128 B contiguous per axis index
+    const int grid = (int)std::min<int64_t>(a.ntiles, grid_cap);
+    fft_strided_kernel<N, T, MODE><<<grid, 16 * T, 0, st>>>(a);
+}
+
+#define RS_DISPATCH_N(N_, FN_, MODE_, ...)                                   \
+    switch (N_) {                                                            \
+    case 16: FN_<16, MODE_>(__VA_ARGS__); break;                             \
+    case 32: FN_<32, MODE_>(__VA_ARGS__); break;                             \
+    case 48: FN_<48, MODE_>(__VA_ARGS__); break;                             \
+    case 64: FN_<64, MODE_>(__VA_ARGS__); break;                             \
+    case 80: FN_<80, MODE_>(__VA_ARGS__); break;                             \
+    case 96: FN_<96, MODE_>(__VA_ARGS__); break;                             \
+    case 112: FN_<112, MODE_>(__VA_ARGS__); break;                           \
+    case 128: FN_<128, MODE_>(__VA_ARGS__); break;                           \
+    default: break;                                                          \
+    }
+
+void launch_lines(int N, int mode, const LinesArgs &a, int cap, cudaStream_t st)
+{
+    if (mode == 0) { RS_DISPATCH_N(N, launch_lines_n, 0, a, cap, st) }
+    else { RS_DISPATCH_N(N, launch_lines_n, 1, a, cap, st) }
+}
+
+void launch_strided(int N, int mode, const StridedArgs &a, int cap, cudaStream_t st)
+{
+    if (mode == 0) { RS_DISPATCH_N(N, launch_strided_n, 0, a, cap, st) }
+    else if (mode == 1) { RS_DISPATCH_N(N, launch_strided_n, 1, a, cap, st) }
+    else { RS_DISPATCH_N(N, launch_strided_n, 2, a, cap, st) }
+}
+
+template <int NP>
+void launch_project_np(const SphereTables &t, const double2 *X, int64_t ldx, int ncol, double dV, double2 *p,
+                       cudaStream_t st)
+{
+    project_kernel<NP><<<dim3(t.natom, ncol), 128, 0, st>>>(t, X, ldx, ncol, dV, p);
+}
+template <int NP>
+void launch_scatter_np(const SphereTables &t, const int32_t *alist, int nlist, const double2 *p, int ncol, double2 *HX,
+                       int64_t ldhx, cudaStream_t st)
+{
+    scatter_kernel<NP, false><<<dim3(nlist, ncol), 128, 0, st>>>(t, alist, p, ncol, HX, ldhx);
+}
+
+SphereTables sphere_tables(const rsdft_plan *P)
+{
+    SphereTables t;
+    t.pt_off = P->pt_off.p; t.beta_off = P->beta_off.p; t.idx = P->idx.p; t.beta = P->beta.p;
+    t.nproj = P->nproj_a.p; t.D = P->Dmat.p; t.natom = P->natom; t.maxproj = P->maxproj;
+    return t;
+}
+
+int default_batch(const rsdft_plan *P)
+{
+    // columns per kernel sequence: keep one batch (X slice + HX slice) well inside the 126 MB L2
+    const int64_t per_col = P->ng * 16;
+    int64_t b = (int64_t)(48ll << 20) / per_col;
+    return (int)std::max<int64_t>(1, std::min<int64_t>(b, 256));
+}
+
+// One batch of columns through the whole operator.
+int apply_h_batch(rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
+{
+    const int Nx = P->n[0], Ny = P->n[1], Nz = P->n[2];
+    const int cap = P->num_sms * 16;
+    const bool nl = P->natom > 0 && P->total_pts > 0;
+    const SphereTables tabs = sphere_tables(P);
+    if (nl) {   // projections read the INPUT orbitals
+        if (P->maxproj <= 4) launch_project_np<4>(tabs, X, ldx, nb, P->dV, P->pq.p, st);
+        else if (P->maxproj <= 9) launch_project_np<9>(tabs, X, ldx, nb, P->dV, P->pq.p, st);
+        else launch_project_np<16>(tabs, X, ldx, nb, P->dV, P->pq.p, st);
+        ++P->last_launches;
+    }
+    LinesArgs la;
+    la.in = X; la.out = HX; la.ld_in = ldx; la.ld_out = ldhx;
+    la.lines_per_col = (int64_t)Nx * Ny; la.nlines = la.lines_per_col * nb;
+    la.tw = P->tw[2].p; la.vloc = P->vloc.p;
+    launch_lines(Nz, 0, la, cap, st);                                     // z forward, X -> HX
+    StridedArgs sy;
+    sy.data = HX; sy.ld = ldhx; sy.inner = Nz; sy.outer = Nx; sy.chunks = Nz / 8;
+    sy.ntiles = (int64_t)nb * sy.outer * sy.chunks; sy.tw = P->tw[1].p; sy.kin_axis = nullptr; sy.kin_inner = nullptr;
+    launch_strided(Ny, 0, sy, cap, st);                                   // y forward
+    StridedArgs sx;
+    sx.data = HX; sx.ld = ldhx; sx.inner = (int64_t)Ny * Nz; sx.outer = 1; sx.chunks = (int)(sx.inner / 8);
+    sx.ntiles = (int64_t)nb * sx.chunks; sx.tw = P->tw[0].p; sx.kin_axis = P->kin_x.p; sx.kin_inner = P->kin_yz.p;
+    launch_strided(Nx, 2, sx, cap, st);                                   // x forward * t(k)/Ng, x inverse
+    launch_strided(Ny, 1, sy, cap, st);                                   // y inverse
+    launch_lines(Nz, 1, la, cap, st);                                     // z inverse + v(r) psi(r)
+    P->last_launches += 5;
+    if (nl) {
+        for (size_t c = 0; c + 1 < P->colour_off.size(); ++c) {
+            const int32_t *al = P->alist.p + P->colour_off[c];
+            const int nlist = P->colour_off[c + 1] - P->colour_off[c];
+            if (nlist == 0) continue;
+            if (P->maxproj <= 4) launch_scatter_np<4>(tabs, al, nlist, P->pq.p, nb, HX, ldhx, st);
+            else if (P->maxproj <= 9) launch_scatter_np<9>(tabs, al, nlist, P->pq.p, nb, HX, ldhx, st);
+            else launch_scatter_np<16>(tabs, al, nlist, P->pq.p, nb, HX, ldhx, st);
+            ++P->last_launches;
+        }
+    }
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
+}
+
+int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
+{
+    const int batch = P->user_batch > 0 ? P->user_batch : default_batch(P);
+    P->batch = batch;
+    if (P->natom > 0) RS_CUDA(P->pq.ensure((size_t)P->natom * P->maxproj * batch));
+    for (int c0 = 0; c0 < ncol; c0 += batch) {
+        const int nb = std::min(batch, ncol - c0);
+        const int rc = apply_h_batch(P, nb, X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx, st);
+        if (rc != RSDFT_OK) return rc;
+    }
+    return RSDFT_OK;
+}
+
+// Gram configuration: 96 x 96 complex tile, 8 warps (2 x 4), each 48 x 24 = 6 x 3 DMMA tiles
+using GCfg = GramCfg<2, 4, 6, 3, 16, 3>;
+constexpr int GRAM_KC = 16;
+
+int choose_kslabs(int64_t ntiles, int64_t nchunks, int sms)
+{
+    // time model: units run in waves of `sms` CTAs; a unit costs its slab length plus a fixed
+    // fill/epilogue overhead (~48 chunks' worth).  Pick the split with the least modelled time.
+    const int64_t ksmax = std::max<int64_t>(1, std::min<int64_t>(64, nchunks / 64));
+    int best = 1;
+    double best_cost = 1e300;
+    for (int64_t ks = 1; ks <= ksmax; ++ks) {
+        const int64_t waves = (ntiles * ks + sms - 1) / sms;
+        const double cost = (double)waves * ((double)((nchunks + ks - 1) / ks) + 48.0);
+        if (cost < best_cost) { best_cost = cost; best = (int)ks; }
+    }
+    return best;
+}
+
+int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2 *HY, int64_t ldhy, double2 *H, double2 *S,
+              int lds, cudaStream_t st)
+{
+    const int tm = (n + GCfg::TM - 1) / GCfg::TM;
+    const int key = n * 4 + (H ? 2 : 0) + (S ? 1 : 0);
+    if (P->gram_tiles_n != key) {
+        std::vector<GramTile> tiles;
+        if (H)
+            for (int i = 0; i < tm; ++i)
+                for (int j = 0; j < tm; ++j) tiles.push_back({(int16_t)i, (int16_t)j, 0, 0});
+        if (S)
+            for (int i = 0; i < tm; ++i)
+                for (int j = i; j < tm; ++j) tiles.push_back({(int16_t)i, (int16_t)j, 1, 0});
+        RS_CUDA(P->gram_tiles.upload(tiles));
+        P->gram_ntiles = (int)tiles.size();
+        P->gram_tiles_n = key;
+    }
+    const int64_t nchunks = P->ng / GRAM_KC;
+    const int ks = choose_kslabs(P->gram_ntiles, nchunks, P->num_sms);
+    RS_CUDA(P->gram_work.ensure((size_t)ks * 2 * n * n));
+    GramArgs a;
+    a.Y = Y; a.HY = HY; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = P->gram_ntiles; a.kslabs = ks;
+    a.nchunks = nchunks; a.tiles = P->gram_tiles.p; a.work = P->gram_work.p;
+    auto kern = gram_dmma_kernel<2, 4, 6, 3, 16, 3>;
+    static thread_local bool attr_set = false;
+    if (!attr_set) {
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
+        attr_set = true;
+    }
+    kern<<<P->gram_ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);
+    GramReduceArgs r;
+    r.work = P->gram_work.p; r.H = H; r.S = S; r.n = n; r.lds = lds; r.kslabs = ks;
+    const int64_t nn = (int64_t)n * n;
+    gram_reduce_kernel<<<(int)std::min<int64_t>((nn + 255) / 256, P->num_sms * 8), 256, 0, st>>>(r);
+    P->last_launches += 2;
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
+}
+
+bool overlaps(const void *a, size_t na, const void *b, size_t nb)
+{
+    const char *pa = (const char *)a, *pb = (const char *)b;
+    return pa < pb + nb && pb < pa + na;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// C ABI
+
+extern "C" {
+
+const char *rsdft_last_error(void) { return g_err.c_str(); }
+
+int rsdft_plan_create(const rsdft_grid_t *grid, const rsdft_box_t *box, const rsdft_atoms_t *atoms,
+                      const rsdft_projectors_t *projectors, rsdft_plan_t **out)
+{
+    if (!grid || !box || !out) return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: null grid/box/out");
+    *out = nullptr;
+    for (int a = 0; a < 3; ++a) {
+        const int N = grid->n[a];
+        if (N <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: grid length <= 0");
+        if (N % 16 != 0 || N > 128)
+            return fail(RSDFT_UNSUPPORTED, "rsdft_plan_create: grid length " + std::to_string(N) +
+                                               " not in {16,32,48,64,80,96,112,128}");
+        if (!(box->len[a] > 0.0) || !std::isfinite(box->len[a]))
+            return fail(RSDFT_UNSUPPORTED, "rsdft_plan_create: box length must be positive and finite");
+    }
+    const bool have_atoms = atoms && atoms->natom > 0 && projectors && projectors->nspecies > 0;
+    if (atoms && atoms->natom < 0) return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: natom < 0");
+    if (atoms && atoms->natom > 0 && (!projectors || projectors->nspecies <= 0 || !projectors->species))
+        return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: atoms given without projectors");
+    if (have_atoms) {
+        if (!atoms->pos || !atoms->species) return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: null atom arrays");
+        for (int s = 0; s < projectors->nspecies; ++s) {
+            const int rc = validate_species(projectors->species[s], box->len, s);
+            if (rc != RSDFT_OK) return rc;
+        }
+        for (int a = 0; a < 3 * atoms->natom; ++a)
+            if (!std::isfinite(atoms->pos[a])) return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: non-finite atom position");
+    }
+    rsdft_plan *P = new (std::nothrow) rsdft_plan();
+    if (!P) return fail(RSDFT_ALLOC, "rsdft_plan_create: host allocation failed");
+    for (int a = 0; a < 3; ++a) { P->n[a] = grid->n[a]; P->len[a] = box->len[a]; }
+    P->ng = (int64_t)P->n[0] * P->n[1] * P->n[2];
+    P->dV = (double)(((long double)P->len[0] / P->n[0]) * ((long double)P->len[1] / P->n[1]) *
+                     ((long double)P->len[2] / P->n[2]));
+    int rc = RSDFT_OK;
+    cudaError_t e = cudaGetDevice(&P->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&P->num_sms, cudaDevAttrMultiProcessorCount, P->device);
+    if (e != cudaSuccess) rc = fail(RSDFT_CUDA, std::string("rsdft_plan_create: ") + cudaGetErrorString(e));
+    try {
+        if (rc == RSDFT_OK) rc = build_fft_tables(P);
+        if (rc == RSDFT_OK && have_atoms) rc = build_spheres(P, atoms, projectors);
+    } catch (const std::bad_alloc &) {
+        rc = fail(RSDFT_ALLOC, "rsdft_plan_create: host allocation failed");
+    }
+    if (rc != RSDFT_OK) { delete P; return rc; }
+    *out = P;
+    return RSDFT_OK;
+}
+
+int rsdft_plan_destroy(rsdft_plan_t *plan)
+{
+    if (!plan) return RSDFT_OK;
+    cudaDeviceSynchronize();
+    delete plan;
+    return RSDFT_OK;
+}
+
+int rsdft_plan_set_vloc(rsdft_plan_t *plan, const double *vloc_dev, void *stream)
+{
+    if (!plan) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_vloc: null plan");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (vloc_dev) RS_CUDA(cudaMemcpyAsync(plan->vloc.p, vloc_dev, plan->vloc.bytes(), cudaMemcpyDeviceToDevice, st));
+    else RS_CUDA(cudaMemsetAsync(plan->vloc.p, 0, plan->vloc.bytes(), st));
+    return RSDFT_OK;
+}
+
+int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols)
+{
+    if (!plan || batch_cols < 0 || batch_cols > 65535) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_batch: bad argument");
+    plan->user_batch = batch_cols;
+    return RSDFT_OK;
+}
+
+int rsdft_plan_info(const rsdft_plan_t *plan, int64_t *out8)
+{
+    if (!plan || !out8) return fail(RSDFT_INVALID_ARG, "rsdft_plan_info: null argument");
+    out8[0] = plan->natom; out8[1] = plan->total_pts; out8[2] = plan->max_pts; out8[3] = (int64_t)plan->device_bytes();
+    out8[4] = plan->user_batch > 0 ? plan->user_batch : default_batch(plan); out8[5] = plan->last_launches;
+    out8[6] = plan->ng; out8[7] = (int64_t)plan->colour_atoms.size();
+    return RSDFT_OK;
+}
+
+int rsdft_apply_h(rsdft_plan_t *plan, int32_t ncol, const void *X, int64_t ldx, void *HX, int64_t ldhx, void *stream)
+{
+    if (!plan || !X || !HX) return fail(RSDFT_INVALID_ARG, "rsdft_apply_h: null argument");
+    if (ncol <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_apply_h: ncol <= 0");
+    if (ldx < plan->ng || ldhx < plan->ng) return fail(RSDFT_INVALID_ARG, "rsdft_apply_h: ld < Ng");
+    if (((uintptr_t)X | (uintptr_t)HX) & 15) return fail(RSDFT_INVALID_ARG, "rsdft_apply_h: pointers must be 16-byte aligned");
+    const size_t bx = ((size_t)(ncol - 1) * ldx + plan->ng) * 16, bh = ((size_t)(ncol - 1) * ldhx + plan->ng) * 16;
+    if (overlaps(X, bx, HX, bh)) return fail(RSDFT_INVALID_ARG, "rsdft_apply_h: X and HX overlap");
+    plan->last_launches = 0;
+    return apply_h_impl(plan, ncol, (const double2 *)X, ldx, (double2 *)HX, ldhx, (cudaStream_t)stream);
+}
+
+int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ldy, const void *HY, int64_t ldhy,
+                        void *H_sub, void *S_sub, int32_t lds, void *stream)
+{
+    if (!plan || !Y) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: null argument");
+    if (n <= 0 || n > 32767 * 96) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: n out of range");
+    if (!H_sub && !S_sub) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: both outputs null");
+    if (H_sub && !HY) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: H_sub requested without HY");
+    if (ldy < plan->ng || (H_sub && ldhy < plan->ng)) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: ld < Ng");
+    if (lds < n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: lds < n");
+    if (((uintptr_t)Y | (uintptr_t)HY | (uintptr_t)H_sub | (uintptr_t)S_sub) & 15)
+        return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: pointers must be 16-byte aligned");
+    plan->last_launches = 0;
+    return gram_impl(plan, n, (const double2 *)Y, ldy, H_sub ? (const double2 *)HY : nullptr, ldhy, (double2 *)H_sub,
+                     (double2 *)S_sub, lds, (cudaStream_t)stream);
+}
+
+int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int64_t ldy, void *HY_host, int64_t ldhy,
+                          void *H_sub_host, void *S_sub_host, int32_t lds)
+{
+    if (!plan || !Y_host || !H_sub_host || !S_sub_host) return fail(RSDFT_INVALID_ARG, "rsdft_block_step_host: null argument");
+    if (n <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_block_step_host: n <= 0");
+    if (ldy < plan->ng || (HY_host && ldhy < plan->ng)) return fail(RSDFT_INVALID_ARG, "rsdft_block_step_host: ld < Ng");
+    if (lds < n) return fail(RSDFT_INVALID_ARG, "rsdft_block_step_host: lds < n");
+    rsdft_plan *P = plan;
+    const int64_t ng = P->ng;
+    RS_CUDA(P->hostY.ensure((size_t)n * ng));
+    RS_CUDA(P->hostHY.ensure((size_t)n * ng));
+    RS_CUDA(P->hostHS.ensure((size_t)2 * n * n));
+    if (!P->s_copy) RS_CUDA(cudaStreamCreateWithFlags(&P->s_copy, cudaStreamNonBlocking));
+    if (!P->s_comp) RS_CUDA(cudaStreamCreateWithFlags(&P->s_comp, cudaStreamNonBlocking));
+    // column chunks of ~256 MB: the H2D copy of chunk k+1 overlaps apply_h on chunk k
+    const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(n, (256ll << 20) / (ng * 16)));
+    const int nchunk = (n + chunk - 1) / chunk;
+    while ((int)P->ev.size() < 2 * nchunk) {
+        cudaEvent_t e;
+        RS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        P->ev.push_back(e);
+    }
+    P->last_launches = 0;
+    for (int k = 0; k < nchunk; ++k) {
+        const int c0 = k * chunk, nc = std::min(chunk, n - c0);
+        RS_CUDA(cudaMemcpy2DAsync(P->hostY.p + (int64_t)c0 * ng, (size_t)ng * 16,
+                                  (const char *)Y_host + (size_t)c0 * ldy * 16, (size_t)ldy * 16, (size_t)ng * 16, nc,
+                                  cudaMemcpyHostToDevice, P->s_copy));
+        RS_CUDA(cudaEventRecord(P->ev[2 * k], P->s_copy));
+        RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev[2 * k], 0));
+        const int rc = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, P->s_comp);
+        if (rc != RSDFT_OK) return rc;
+        RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], P->s_comp));
+    }
+    const int64_t launches = P->last_launches;
+    double2 *Hd = P->hostHS.p, *Sd = P->hostHS.p + (size_t)n * n;
+    int rc = gram_impl(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->s_comp);
+    if (rc != RSDFT_OK) return rc;
+    P->last_launches += launches;
+    RS_CUDA(cudaMemcpy2DAsync(H_sub_host, (size_t)lds * 16, Hd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
+    RS_CUDA(cudaMemcpy2DAsync(S_sub_host, (size_t)lds * 16, Sd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
+    if (HY_host) {   // HY goes back on the copy stream, behind the uploads, while the Gram runs
+        for (int k = 0; k < nchunk; ++k) {
+            const int c0 = k * chunk, nc = std::min(chunk, n - c0);
+            RS_CUDA(cudaStreamWaitEvent(P->s_copy, P->ev[2 * k + 1], 0));
+            RS_CUDA(cudaMemcpy2DAsync((char *)HY_host + (size_t)c0 * ldhy * 16, (size_t)ldhy * 16,
+                                      P->hostHY.p + (int64_t)c0 * ng, (size_t)ng * 16, (size_t)ng * 16, nc,
+                                      cudaMemcpyDeviceToHost, P->s_copy));
+        }
+    }
+    RS_CUDA(cudaStreamSynchronize(P->s_comp));
+    RS_CUDA(cudaStreamSynchronize(P->s_copy));
+    return RSDFT_OK;
+}
+
+}  // extern "C"

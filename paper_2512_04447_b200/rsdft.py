@@ -1,0 +1,259 @@
+"""Thin ctypes binding over librsdft.so (include/rsdft.h) -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; there is no CPU fallback:
+if the library is missing, or it reports an error, the call raises.  torch is used for device
+memory and streams only (torch tensors' data_ptr() / torch.cuda.current_stream()).
+
+Function names follow the C ABI: rsdft_plan_create, rsdft_plan_set_vloc, rsdft_apply_h,
+rsdft_subspace_gram, rsdft_block_step_host, rsdft_plan_info, rsdft_plan_set_batch,
+rsdft_plan_destroy, rsdft_last_error.  Orbital blocks are torch complex128 tensors of shape
+[ncol, ld] (row c = column c of the paper's block, contiguous in the grid index)."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librsdft.so")
+
+SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram",
+           "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_destroy",
+           "rsdft_last_error"]
+
+RSDFT_OK, RSDFT_INVALID_ARG, RSDFT_UNSUPPORTED, RSDFT_ALLOC, RSDFT_CUDA = 0, -1, -2, -3, -4
+
+
+class RsdftError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("librsdft error %d: %s" % (code, msg))
+        self.code = code
+
+
+class _Grid(C.Structure):
+    _fields_ = [("n", C.c_int32 * 3)]
+
+
+class _Box(C.Structure):
+    _fields_ = [("len", C.c_double * 3)]
+
+
+class _Atoms(C.Structure):
+    _fields_ = [("natom", C.c_int32), ("pos", C.POINTER(C.c_double)), ("species", C.POINTER(C.c_int32))]
+
+
+class _Species(C.Structure):
+    _fields_ = [("rc", C.c_double), ("nproj", C.c_int32),
+                ("l", C.POINTER(C.c_int32)), ("m", C.POINTER(C.c_int32)),
+                ("radial_kind", C.c_int32), ("alpha", C.POINTER(C.c_double)),
+                ("nr", C.c_int32), ("dr", C.c_double), ("radial", C.POINTER(C.c_double)),
+                ("D", C.POINTER(C.c_double))]
+
+
+class _Projectors(C.Structure):
+    _fields_ = [("nspecies", C.c_int32), ("species", C.POINTER(_Species))]
+
+
+_lib = None
+
+
+def load():
+    """dlopen librsdft.so; raises (never falls back) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("librsdft.so is not built: run `python -m paper_2512_04447_b200.build` "
+                           "(there is no CPU fallback for the CUDA path)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    lib.rsdft_plan_create.argtypes = [C.POINTER(_Grid), C.POINTER(_Box), C.POINTER(_Atoms),
+                                      C.POINTER(_Projectors), C.POINTER(vp)]
+    lib.rsdft_plan_set_vloc.argtypes = [vp, vp, vp]
+    lib.rsdft_apply_h.argtypes = [vp, i32, vp, i64, vp, i64, vp]
+    lib.rsdft_subspace_gram.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32, vp]
+    lib.rsdft_block_step_host.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32]
+    lib.rsdft_plan_info.argtypes = [vp, C.POINTER(i64)]
+    lib.rsdft_plan_set_batch.argtypes = [vp, i32]
+    lib.rsdft_plan_destroy.argtypes = [vp]
+    lib.rsdft_last_error.restype = C.c_char_p
+    for name in SYMBOLS:
+        if name != "rsdft_last_error":
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def rsdft_last_error():
+    return load().rsdft_last_error().decode()
+
+
+def _check(rc):
+    if rc != RSDFT_OK:
+        raise RsdftError(rc, rsdft_last_error())
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _ip(a):
+    return a.ctypes.data_as(C.POINTER(C.c_int32))
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    return C.c_void_p(int(stream))
+
+
+class Plan:
+    """Owner of an rsdft_plan_t* (destroyed on close() / garbage collection)."""
+
+    def __init__(self, handle, n, length):
+        self.handle = handle
+        self.n = tuple(n)
+        self.len = tuple(length)
+        self.ng = int(n[0]) * int(n[1]) * int(n[2])
+
+    def close(self):
+        if self.handle:
+            load().rsdft_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def rsdft_plan_create(grid, box, atoms=None, projectors=None):
+    """grid: (Nx, Ny, Nz); box: (Lx, Ly, Lz) bohr; atoms: (pos[natom,3], species_of[natom]) or
+    None; projectors: list of species dicts {rc, l, m, D, radial_kind, alpha | (dr, radial)}."""
+    lib = load()
+    g = _Grid((C.c_int32 * 3)(*[int(v) for v in grid]))
+    b = _Box((C.c_double * 3)(*[float(v) for v in box]))
+    keep = []
+    a_ptr = p_ptr = None
+    if atoms is not None:
+        pos = np.ascontiguousarray(atoms[0], dtype=np.float64).reshape(-1, 3)
+        spo = np.ascontiguousarray(atoms[1], dtype=np.int32).reshape(-1)
+        if spo.shape[0] != pos.shape[0]:
+            raise ValueError("species_of and pos disagree on natom")
+        keep += [pos, spo]
+        a_ptr = C.pointer(_Atoms(pos.shape[0], _dp(pos), _ip(spo)))
+    if projectors is not None:
+        arr = (_Species * max(1, len(projectors)))()
+        for s, sp in enumerate(projectors):
+            l = np.ascontiguousarray(sp["l"], dtype=np.int32)
+            m = np.ascontiguousarray(sp["m"], dtype=np.int32)
+            D = np.ascontiguousarray(sp["D"], dtype=np.float64)
+            nproj = int(l.shape[0])
+            alpha = np.ascontiguousarray(sp.get("alpha", np.zeros(nproj)), dtype=np.float64)
+            radial = np.ascontiguousarray(sp.get("radial", np.zeros((nproj, 2))), dtype=np.float64)
+            keep += [l, m, D, alpha, radial]
+            arr[s] = _Species(float(sp["rc"]), nproj, _ip(l), _ip(m), int(sp.get("radial_kind", 0)), _dp(alpha),
+                              int(radial.shape[1]), float(sp.get("dr", 1.0)), _dp(radial), _dp(D))
+        keep.append(arr)
+        p_ptr = C.pointer(_Projectors(len(projectors), arr))
+    out = C.c_void_p()
+    _check(lib.rsdft_plan_create(C.byref(g), C.byref(b), a_ptr, p_ptr, C.byref(out)))
+    return Plan(out, grid, box)
+
+
+def plan_from_system(system):
+    """Convenience: plan for a workloads.make_system() dict, V_loc uploaded if present."""
+    import torch
+    natom = len(system.get("pos", []))
+    plan = rsdft_plan_create(system["n"], system["len"],
+                             (system["pos"], system["species_of"]) if natom else None,
+                             system["species"] if natom else None)
+    if system.get("vloc") is not None:
+        v = torch.as_tensor(np.ascontiguousarray(system["vloc"], dtype=np.float64)).cuda()
+        rsdft_plan_set_vloc(plan, v)
+        torch.cuda.current_stream().synchronize()
+    return plan
+
+
+def rsdft_plan_set_vloc(plan, vloc, stream=None):
+    """vloc: torch float64 CUDA tensor [Ng], or None to reset V_loc to 0."""
+    ptr = None
+    if vloc is not None:
+        if not (vloc.is_cuda and vloc.is_contiguous() and vloc.numel() == plan.ng and vloc.element_size() == 8):
+            raise ValueError("vloc must be a contiguous float64 CUDA tensor of Ng elements")
+        ptr = C.c_void_p(vloc.data_ptr())
+    _check(load().rsdft_plan_set_vloc(plan.handle, ptr, _stream(stream)))
+
+
+def _block(t, name):
+    import torch
+    if not (t.is_cuda and t.dtype == torch.complex128 and t.dim() == 2 and t.stride(1) == 1):
+        raise ValueError("%s must be a CUDA complex128 tensor [ncol, ld] with unit inner stride" % name)
+    return t.shape[0], (t.stride(0) if t.shape[0] > 1 else max(t.shape[1], t.stride(0)))
+
+
+def rsdft_apply_h(plan, X, HX, stream=None):
+    """HX[c, :Ng] = (T + V_loc + V_NL) X[c, :Ng] for every row c.  X, HX: [ncol, ld] CUDA complex128."""
+    ncol, ldx = _block(X, "X")
+    ncol2, ldhx = _block(HX, "HX")
+    if ncol != ncol2:
+        raise ValueError("X and HX disagree on ncol")
+    _check(load().rsdft_apply_h(plan.handle, ncol, C.c_void_p(X.data_ptr()), ldx, C.c_void_p(HX.data_ptr()), ldhx,
+                                _stream(stream)))
+    return HX
+
+
+def rsdft_subspace_gram(plan, Y, HY, H_sub=None, S_sub=None, stream=None, want_h=True, want_s=True):
+    """-> (H_sub, S_sub) as torch [n, n] complex128 CUDA tensors holding the COLUMN-MAJOR
+    matrices: M_store[j, i] = M[i, j] (so M = M_store.T).  Y, HY: [n, ld]."""
+    import torch
+    n, ldy = _block(Y, "Y")
+    ldhy = ldy
+    if want_h:
+        n2, ldhy = _block(HY, "HY")
+        if n2 != n:
+            raise ValueError("Y and HY disagree on n")
+    if want_h and H_sub is None:
+        H_sub = torch.empty((n, n), dtype=torch.complex128, device=Y.device)
+    if want_s and S_sub is None:
+        S_sub = torch.empty((n, n), dtype=torch.complex128, device=Y.device)
+    _check(load().rsdft_subspace_gram(plan.handle, n, C.c_void_p(Y.data_ptr()), ldy,
+                                      C.c_void_p(HY.data_ptr()) if want_h else None, ldhy,
+                                      C.c_void_p(H_sub.data_ptr()) if want_h else None,
+                                      C.c_void_p(S_sub.data_ptr()) if want_s else None, n, _stream(stream)))
+    return H_sub, S_sub
+
+
+def rsdft_block_step_host(plan, Y_host, HY_host=None, H_sub_host=None, S_sub_host=None):
+    """One whole block step from HOST tensors (pinned recommended): uploads Y in chunks overlapped
+    with apply_h, forms the Gram matrices, downloads them (and HY if HY_host is given)."""
+    import torch
+    if Y_host.is_cuda or Y_host.dtype != torch.complex128 or Y_host.dim() != 2 or Y_host.stride(1) != 1:
+        raise ValueError("Y_host must be a host complex128 tensor [n, ld]")
+    n, ldy = Y_host.shape[0], Y_host.stride(0)
+    if H_sub_host is None:
+        H_sub_host = torch.empty((n, n), dtype=torch.complex128).pin_memory()
+    if S_sub_host is None:
+        S_sub_host = torch.empty((n, n), dtype=torch.complex128).pin_memory()
+    _check(load().rsdft_block_step_host(plan.handle, n, C.c_void_p(Y_host.data_ptr()), ldy,
+                                        C.c_void_p(HY_host.data_ptr()) if HY_host is not None else None,
+                                        HY_host.stride(0) if HY_host is not None else 0,
+                                        C.c_void_p(H_sub_host.data_ptr()), C.c_void_p(S_sub_host.data_ptr()), n))
+    return H_sub_host, S_sub_host
+
+
+def rsdft_plan_info(plan):
+    out = (C.c_int64 * 8)()
+    _check(load().rsdft_plan_info(plan.handle, out))
+    keys = ["natom", "sphere_points", "max_sphere_points", "device_bytes", "batch_cols", "last_launches", "ng",
+            "colour_classes"]
+    return dict(zip(keys, [int(v) for v in out]))
+
+
+def rsdft_plan_set_batch(plan, batch_cols):
+    _check(load().rsdft_plan_set_batch(plan.handle, int(batch_cols)))
+
+
+def rsdft_plan_destroy(plan):
+    plan.close()

@@ -1,0 +1,235 @@
+"""GPU parity: the CUDA path through the C ABI vs the CPU oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star; R16): max_g |gpu - oracle| / max_g |oracle| <= 1e-12 per
+column for HX, per matrix for H_sub and S_sub, complex128.  Integer work (sphere point counts)
+is compared exactly.  Every test here needs a B200 (pytest -m gpu)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from oracle import oracle
+    from paper_2512_04447_b200 import rsdft, workloads
+    assert torch.cuda.is_available()
+    rsdft.load()          # fails loudly if the extension is missing
+    return dict(torch=torch, oracle=oracle, rsdft=rsdft, wl=workloads)
+
+
+def col_err(gpu, ref):
+    """per-row normwise error of [ncol, Ng] arrays"""
+    num = np.max(np.abs(gpu - ref), axis=1)
+    den = np.max(np.abs(ref), axis=1)
+    return float(np.max(num / den))
+
+
+def mat_err(gpu, ref):
+    return float(np.max(np.abs(gpu - ref)) / np.max(np.abs(ref)))
+
+
+def blocks(env, system, cols_per_block=None, ld=None):
+    """X, W, P seeded blocks (streams 0, 1, 2) stacked into Y [3m, ld] on the device."""
+    wl, torch = env["wl"], env["torch"]
+    m = system["m"] if cols_per_block is None else cols_per_block
+    ng = int(np.prod(system["n"]))
+    return torch.cat([wl.orbital_block(ng, range(m), system["seed"], s, device="cuda", ld=ld) for s in range(3)], dim=0)
+
+
+def gpu_apply(env, plan, X):
+    torch, rsdft = env["torch"], env["rsdft"]
+    HX = torch.full_like(X, float("nan"))
+    rsdft.rsdft_apply_h(plan, X, HX)
+    torch.cuda.synchronize()
+    return HX
+
+
+# ------------------------------------------------------------------ configs 0 and 1, everything
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_block_step_parity_full(env, cfg):
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    system = wl.make_system(cfg)
+    ng = int(np.prod(system["n"]))
+    plan = rsdft.plan_from_system(system)
+    info = rsdft.rsdft_plan_info(plan)
+    Y = blocks(env, system)
+    HY = gpu_apply(env, plan, Y)
+    Yh = Y.cpu().numpy()
+    HY_ref, p_ref = oracle.apply_h(system, Yh, return_p=True)
+    assert col_err(HY.cpu().numpy(), HY_ref) <= TOL
+    # integer work: sphere sizes agree exactly with the oracle's all-grid scan
+    npts = sum(len(oracle.sphere(system["n"], system["len"], R, system["species"][0])[0]) for R in system["pos"])
+    assert info["sphere_points"] == npts and info["ng"] == ng
+    H, S = rsdft.rsdft_subspace_gram(plan, Y, HY)
+    torch.cuda.synchronize()
+    H_ref, S_ref = oracle.gram(Yh, HY_ref)
+    Hg, Sg = H.cpu().numpy().T, S.cpu().numpy().T          # column-major storage -> M[i, j]
+    assert mat_err(Hg, H_ref) <= TOL
+    assert mat_err(Sg, S_ref) <= TOL
+    assert np.array_equal(Sg, Sg.conj().T)                  # exactly Hermitian
+    assert np.all(np.diagonal(Sg).imag == 0.0)
+    assert mat_err(Hg, Hg.conj().T) <= 1e-13                # Hermitian to round-off
+    np.linalg.cholesky(Sg)                                  # positive definite
+    plan.close()
+
+
+def test_apply_h_only_x_block_config0(env):
+    """configs[0]: 'one rsdft_apply_h on X' (8 columns)."""
+    oracle, rsdft, wl = env["oracle"], env["rsdft"], env["wl"]
+    system = wl.make_system(0)
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(4096, range(8), 0, 0, device="cuda")
+    HX = gpu_apply(env, plan, X)
+    assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
+
+
+# ------------------------------------------------------------------ every supported length on every axis
+@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 112, 128])
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_kinetic_every_length_every_axis(env, N, axis):
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    n = [16, 16, 16]
+    n[axis] = N
+    L = [6.0, 7.0, 8.0]
+    L[axis] = 0.31 * N
+    ng = int(np.prod(n))
+    rng = np.random.default_rng(100 + N + axis)
+    system = dict(n=tuple(n), len=tuple(L), vloc=rng.standard_normal(ng))
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(ng, range(3), 77, axis, device="cuda")
+    HX = gpu_apply(env, plan, X)
+    assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
+    # plane wave with negative frequency along `axis` is an eigenvector of T (V_loc = 0)
+    rsdft.rsdft_plan_set_vloc(plan, None)
+    k = N - 3
+    idx = np.indices(n)[axis].reshape(-1)
+    pw = torch.as_tensor(np.exp(2j * np.pi * k * idx / N)[None, :]).cuda()
+    Tpw = gpu_apply(env, plan, pw).cpu().numpy()
+    lam = 0.5 * (2 * np.pi * (k - N) / L[axis]) ** 2
+    # round-off in the empty Fourier modes is amplified by their own t(k): scale by max_k t(k)
+    tmax = 0.5 * sum((np.pi * n[a] / L[a]) ** 2 for a in range(3))
+    assert np.max(np.abs(Tpw - lam * pw.cpu().numpy())) <= 1e-13 * tmax
+
+
+# ------------------------------------------------------------------ degenerate / ragged inputs
+def test_no_atoms_no_vloc_is_kinetic_only(env):
+    oracle, rsdft, wl = env["oracle"], env["rsdft"], env["wl"]
+    system = dict(n=(32, 16, 48), len=(9.0, 5.0, 13.0), vloc=None)
+    plan = rsdft.rsdft_plan_create(system["n"], system["len"])
+    ng = 32 * 16 * 48
+    X = wl.orbital_block(ng, range(5), 5, 0, device="cuda")
+    HX = gpu_apply(env, plan, X)
+    assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
+    assert rsdft.rsdft_plan_info(plan)["natom"] == 0
+
+
+@pytest.mark.parametrize("radial_kind", [0, 1])
+def test_noncubic_spd_projectors_full_D_padded_ld(env, radial_kind):
+    """9 s+p+d projectors, full symmetric D, tabulated radial part, overlapping spheres, ld > Ng,
+    ncol not a multiple of the batch width; result independent of the batch width (bitwise)."""
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    system = wl.small_system(n=(32, 16, 48), L=(7.0, 4.1, 9.5), natom=5, seed=11, nproj=9, rc=1.9,
+                             radial_kind=radial_kind)
+    ng = 32 * 16 * 48
+    plan = rsdft.plan_from_system(system)
+    assert rsdft.rsdft_plan_info(plan)["colour_classes"] >= 2          # spheres do overlap here
+    X = wl.orbital_block(ng, range(7), 3, 0, device="cuda", ld=ng + 24)
+    ref = oracle.apply_h(system, X[:, :ng].cpu().numpy())
+    outs = []
+    for batch in (0, 1, 3, 7, 16):
+        rsdft.rsdft_plan_set_batch(plan, batch)
+        HX = gpu_apply(env, plan, X)
+        assert col_err(HX[:, :ng].cpu().numpy(), ref) <= TOL
+        assert bool(torch.isnan(HX[:, ng:].real).all())                 # padding untouched
+        outs.append(HX[:, :ng].clone())
+    for o in outs[1:]:
+        assert torch.equal(torch.view_as_real(o), torch.view_as_real(outs[0]))
+
+
+def test_single_column_and_sphere_wrapping(env):
+    """One column; atoms placed at the box corner and outside [0, L) so spheres wrap periodically."""
+    oracle, rsdft, wl = env["oracle"], env["rsdft"], env["wl"]
+    system = wl.small_system(n=(16, 16, 16), L=(5.0, 5.0, 5.0), natom=3, seed=5, nproj=4, rc=1.7)
+    system["pos"] = np.array([[0.01, 0.02, 4.99], [-1.3, 6.2, 2.5], [2.5, 2.5, 2.5]])
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(4096, [0], 9, 0, device="cuda")
+    HX = gpu_apply(env, plan, X)
+    assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
+
+
+@pytest.mark.parametrize("n", [1, 7, 96, 97, 200])
+def test_gram_ragged_sizes_and_options(env, n):
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    plan = rsdft.rsdft_plan_create((16, 32, 16), (5.0, 9.0, 5.0))
+    ng = 16 * 32 * 16
+    Y = wl.orbital_block(ng, range(n), 21, 0, device="cuda", ld=ng + 8)
+    HY = wl.orbital_block(ng, range(n), 21, 1, device="cuda")
+    H_ref, S_ref = oracle.gram(Y[:, :ng].cpu().numpy(), HY.cpu().numpy())
+    H, S = rsdft.rsdft_subspace_gram(plan, Y, HY)
+    torch.cuda.synchronize()
+    assert mat_err(H.cpu().numpy().T, H_ref) <= TOL
+    assert mat_err(S.cpu().numpy().T, S_ref) <= TOL
+    _, S2 = rsdft.rsdft_subspace_gram(plan, Y, None, want_h=False)
+    H2, _ = rsdft.rsdft_subspace_gram(plan, Y, HY, want_s=False)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(S2), torch.view_as_real(S))    # deterministic, bitwise
+    assert torch.equal(torch.view_as_real(H2), torch.view_as_real(H))
+
+
+def test_gram_plane_waves_closed_form(env):
+    """Plane-wave columns: S_sub = Ng I, H_sub = Ng diag(t) (V = 0, no projectors) -- closed form."""
+    torch, rsdft = env["torch"], env["rsdft"]
+    n, L = (16, 16, 32), (10.0, 10.0, 12.0)
+    ng = int(np.prod(n))
+    plan = rsdft.rsdft_plan_create(n, L)
+    ks = [(0, 0, 0), (1, 0, 0), (0, 15, 0), (0, 0, 16), (3, 2, 31), (8, 8, 1)]
+    ii = np.indices(n).reshape(3, -1)
+    Y = np.stack([np.exp(2j * np.pi * sum(k[a] * ii[a] / n[a] for a in range(3))) for k in ks])
+    Yd = torch.as_tensor(Y).cuda()
+    HY = gpu_apply(env, plan, Yd)
+    H, S = rsdft.rsdft_subspace_gram(plan, Yd, HY)
+    torch.cuda.synchronize()
+    kap = lambda j, N: j if 2 * j < N else j - N
+    t = np.array([0.5 * sum((2 * np.pi * kap(k[a], n[a]) / L[a]) ** 2 for a in range(3)) for k in ks])
+    assert np.max(np.abs(S.cpu().numpy().T - ng * np.eye(len(ks)))) <= 1e-12 * ng
+    assert np.max(np.abs(H.cpu().numpy().T - ng * np.diag(t))) <= 1e-12 * ng * t.max()
+
+
+def test_error_paths_on_device(env):
+    torch, rsdft = env["torch"], env["rsdft"]
+    plan = rsdft.rsdft_plan_create((16, 16, 16), (10.0,) * 3)
+    X = torch.zeros((2, 4096), dtype=torch.complex128, device="cuda")
+    with pytest.raises(rsdft.RsdftError) as e:
+        rsdft.rsdft_apply_h(plan, X, X)                                   # aliasing
+    assert e.value.code == rsdft.RSDFT_INVALID_ARG and "overlap" in str(e.value)
+    short = torch.zeros((2, 4000), dtype=torch.complex128, device="cuda")
+    with pytest.raises(rsdft.RsdftError):
+        rsdft.rsdft_apply_h(plan, short, torch.zeros_like(short))         # ld < Ng
+    with pytest.raises(rsdft.RsdftError):
+        rsdft.rsdft_subspace_gram(plan, short, short)
+    with pytest.raises(ValueError):
+        rsdft.rsdft_apply_h(plan, X.cpu(), X)                             # host tensor
+    lib = rsdft.load()
+    assert lib.rsdft_apply_h(plan.handle, 0, X.data_ptr(), 4096, X.data_ptr(), 4096, None) == rsdft.RSDFT_INVALID_ARG
+
+
+def test_block_step_host_matches_device_path(env):
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    system = wl.make_system(1)
+    ng = 48 ** 3
+    plan = rsdft.plan_from_system(system)
+    Y = blocks(env, system, cols_per_block=8)
+    Yh = Y.cpu().pin_memory()
+    HYh = torch.empty_like(Yh).pin_memory()
+    H, S = rsdft.rsdft_block_step_host(plan, Yh, HYh)
+    HY_ref = oracle.apply_h(system, Yh.numpy())
+    H_ref, S_ref = oracle.gram(Yh.numpy(), HY_ref)
+    assert col_err(HYh.numpy(), HY_ref) <= TOL
+    assert mat_err(H.numpy().T, H_ref) <= TOL and mat_err(S.numpy().T, S_ref) <= TOL
+    HY = gpu_apply(env, plan, Y)
+    assert torch.equal(torch.view_as_real(HY.cpu()), torch.view_as_real(HYh))
+    assert rsdft.rsdft_plan_info(plan)["last_launches"] > 0
