@@ -12,6 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librsdft.so")
+PROBE_LIB = os.path.join(HERE, "libpeakprobe.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 
@@ -22,14 +23,19 @@ def sources():
     return deps
 
 
+def _stale(lib, deps, force):
+    return force or not os.path.exists(lib) or any(os.path.getmtime(lib) < os.path.getmtime(d) for d in deps)
+
+
 def build(force=False, verbose=False):
-    """Compile csrc/rsdft.cu -> librsdft.so if any source is newer than the library."""
-    deps = sources()
-    if (not force) and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
-        return LIB
+    """Compile csrc/rsdft.cu -> librsdft.so (the product) and csrc/peak_probe.cu -> libpeakprobe.so
+    (bench.py's roofline-denominator probe) if any source is newer than the library."""
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB, os.path.join(CSRC, "rsdft.cu")]
-    subprocess.check_call(cmd)
+    extra = ["-Xptxas", "-v"] if verbose else []
+    if _stale(LIB, [d for d in sources() if not d.endswith("peak_probe.cu")], force):
+        subprocess.check_call([nvcc] + NVCC_FLAGS + extra + ["-o", LIB, os.path.join(CSRC, "rsdft.cu")])
+    if _stale(PROBE_LIB, [os.path.join(CSRC, "peak_probe.cu")], force):
+        subprocess.check_call([nvcc] + NVCC_FLAGS + extra + ["-o", PROBE_LIB, os.path.join(CSRC, "peak_probe.cu")])
     return LIB
 
 
