@@ -14,7 +14,7 @@
 #include <string>
 #include <vector>
 
-#include "fft_kernels.cuh"
+#include "fft3_kernels.cuh"
 #include "gram_kernels.cuh"
 #include "nonlocal_kernels.cuh"
 
@@ -80,7 +80,7 @@ struct rsdft_plan {
     // FFT tables
     DevBuf<double2> tw[3];        // per axis: w_N^m = (cos, -sin)(2 pi m / N)
     DevBuf<double> kin_x;         // t_x[kx] / Ng                       [Nx]
-    DevBuf<double> kin_yz;        // (t_y[ky] + t_z[kz]) / Ng           [Ny*Nz]
+    DevBuf<double> kin_yz;        // (t_y[ky(r)] + t_z[kz(p)]) / Ng at r*Nz + p, permuted positions (fft3_kernels.cuh)
     DevBuf<double> vloc;          // [Ng], zero until set
 
     // projector tables
@@ -318,8 +318,14 @@ int build_fft_tables(rsdft_plan *P)
     };
     std::vector<double> kx(P->n[0]), kyz((size_t)P->n[1] * P->n[2]);
     for (int i = 0; i < P->n[0]; ++i) kx[i] = (double)(t_axis(0, i) * inv_ng);
-    for (int j = 0; j < P->n[1]; ++j)
-        for (int k = 0; k < P->n[2]; ++k) kyz[(size_t)j * P->n[2] + k] = (double)((t_axis(1, j) + t_axis(2, k)) * inv_ng);
+    // k-space positions are permuted by the in-place transforms: y row r = k1*My + k2 holds ky = k1 + 16*k2
+    // ("16-first"), z position p = k1*16 + k2 holds kz = k1 + Mz*k2 ("M-first"); x is indexed naturally.
+    const int My = P->n[1] / 16, Mz = P->n[2] / 16;
+    for (int r = 0; r < P->n[1]; ++r)
+        for (int p = 0; p < P->n[2]; ++p) {
+            const int ky = r / My + 16 * (r % My), kz = p / 16 + Mz * (p % 16);
+            kyz[(size_t)r * P->n[2] + p] = (double)((t_axis(1, ky) + t_axis(2, kz)) * inv_ng);
+        }
     RS_CUDA(P->kin_x.upload(kx));
     RS_CUDA(P->kin_yz.upload(kyz));
     RS_CUDA(P->vloc.alloc((size_t)P->ng));
@@ -336,47 +342,76 @@ namespace {
 
 using namespace rsdft;
 
-template <int N, int MODE>
-void launch_lines_n(const LinesArgs &a, int grid_cap, cudaStream_t st)
-{
-    constexpr int L = 8;   // 128 threads, 8 contiguous lines per CTA
-    const int64_t blocks = (a.nlines + L - 1) / L;
-    const int grid = (int)std::min<int64_t>(blocks, grid_cap);
-    fft_lines_kernel<N, L, MODE><<<grid, 16 * L, 0, st>>>(a);
-}
-
-template <int N, int MODE>
-void launch_strided_n(const StridedArgs &a, int grid_cap, cudaStream_t st)
-{
-    constexpr int T = 8;   // 128 threads, 128 B contiguous per axis index
-    const int grid = (int)std::min<int64_t>(a.ntiles, grid_cap);
-    fft_strided_kernel<N, T, MODE><<<grid, 16 * T, 0, st>>>(a);
-}
-
-#define RS_DISPATCH_N(N_, FN_, MODE_, ...)                                   \
+#define RS_DISPATCH_N(N_, FN_, ...)                                          \
     switch (N_) {                                                            \
-    case 16: FN_<16, MODE_>(__VA_ARGS__); break;                             \
-    case 32: FN_<32, MODE_>(__VA_ARGS__); break;                             \
-    case 48: FN_<48, MODE_>(__VA_ARGS__); break;                             \
-    case 64: FN_<64, MODE_>(__VA_ARGS__); break;                             \
-    case 80: FN_<80, MODE_>(__VA_ARGS__); break;                             \
-    case 96: FN_<96, MODE_>(__VA_ARGS__); break;                             \
-    case 112: FN_<112, MODE_>(__VA_ARGS__); break;                           \
-    case 128: FN_<128, MODE_>(__VA_ARGS__); break;                           \
+    case 16: FN_<16>(__VA_ARGS__); break;                                    \
+    case 32: FN_<32>(__VA_ARGS__); break;                                    \
+    case 48: FN_<48>(__VA_ARGS__); break;                                    \
+    case 64: FN_<64>(__VA_ARGS__); break;                                    \
+    case 80: FN_<80>(__VA_ARGS__); break;                                    \
+    case 96: FN_<96>(__VA_ARGS__); break;                                    \
+    case 112: FN_<112>(__VA_ARGS__); break;                                  \
+    case 128: FN_<128>(__VA_ARGS__); break;                                  \
     default: break;                                                          \
     }
 
-void launch_lines(int N, int mode, const LinesArgs &a, int cap, cudaStream_t st)
+// grid of the zy / yz kernels: G plane-walkers for each of the my row classes
+inline int rows_grid(const Fft3Args &a, int sms)
 {
-    if (mode == 0) { RS_DISPATCH_N(N, launch_lines_n, 0, a, cap, st) }
-    else { RS_DISPATCH_N(N, launch_lines_n, 1, a, cap, st) }
+    const int64_t planes = (int64_t)a.ncol * a.nx;
+    const int64_t g = std::max<int64_t>(1, std::min<int64_t>(planes, (int64_t)sms * 8 / a.my));
+    return (int)(g * a.my);
 }
 
-void launch_strided(int N, int mode, const StridedArgs &a, int cap, cudaStream_t st)
+template <int NZ>
+void launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    if (mode == 0) { RS_DISPATCH_N(N, launch_strided_n, 0, a, cap, st) }
-    else if (mode == 1) { RS_DISPATCH_N(N, launch_strided_n, 1, a, cap, st) }
-    else { RS_DISPATCH_N(N, launch_strided_n, 2, a, cap, st) }
+    fft3_fwd_zy_kernel<NZ><<<rows_grid(a, sms), 128, 0, st>>>(a);
+}
+template <int NZ>
+void launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    fft3_inv_yz_kernel<NZ><<<rows_grid(a, sms), 128, 0, st>>>(a);
+}
+
+constexpr int FFT3_TZ = 8;      // z points per x-kernel tile: 128 B contiguous per (x, row)
+
+template <int NX>
+cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    const size_t smem = (size_t)NX * (a.my * FFT3_TZ + 1) * sizeof(double2);
+    const int64_t ntiles = (int64_t)a.ncol * 16 * (a.nz / FFT3_TZ);
+    cudaError_t e;
+    if (2 * (smem + 4096) <= 227 * 1024) {
+        auto k = fft3_x_kernel<NX, FFT3_TZ, 256, 2>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        const int occ = (int)std::min<size_t>(2, (227 * 1024) / (smem + 4096));
+        k<<<(int)std::min<int64_t>(ntiles, (int64_t)sms * occ), 256, smem, st>>>(a);
+    } else {
+        auto k = fft3_x_kernel<NX, FFT3_TZ, 512, 1>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k<<<(int)std::min<int64_t>(ntiles, sms), 512, smem, st>>>(a);
+    }
+    return cudaSuccess;
+}
+
+cudaError_t launch_x_any(int nx, const Fft3Args &a, int sms, cudaStream_t st)
+{
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (nx) {
+    case 16: e = launch_x<16>(a, sms, st); break;
+    case 32: e = launch_x<32>(a, sms, st); break;
+    case 48: e = launch_x<48>(a, sms, st); break;
+    case 64: e = launch_x<64>(a, sms, st); break;
+    case 80: e = launch_x<80>(a, sms, st); break;
+    case 96: e = launch_x<96>(a, sms, st); break;
+    case 112: e = launch_x<112>(a, sms, st); break;
+    case 128: e = launch_x<128>(a, sms, st); break;
+    default: break;
+    }
+    return e;
 }
 
 template <int NP>
@@ -412,7 +447,6 @@ int default_batch(const rsdft_plan *P)
 int apply_h_batch(rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
 {
     const int Nx = P->n[0], Ny = P->n[1], Nz = P->n[2];
-    const int cap = P->num_sms * 16;
     const bool nl = P->natom > 0 && P->total_pts > 0;
     const SphereTables tabs = sphere_tables(P);
     if (nl) {   // projections read the INPUT orbitals
@@ -421,22 +455,15 @@ int apply_h_batch(rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 
         else launch_project_np<16>(tabs, X, ldx, nb, P->dV, P->pq.p, st);
         ++P->last_launches;
     }
-    LinesArgs la;
-    la.in = X; la.out = HX; la.ld_in = ldx; la.ld_out = ldhx;
-    la.lines_per_col = (int64_t)Nx * Ny; la.nlines = la.lines_per_col * nb;
-    la.tw = P->tw[2].p; la.vloc = P->vloc.p;
-    launch_lines(Nz, 0, la, cap, st);                                     // z forward, X -> HX
-    StridedArgs sy;
-    sy.data = HX; sy.ld = ldhx; sy.inner = Nz; sy.outer = Nx; sy.chunks = Nz / 8;
-    sy.ntiles = (int64_t)nb * sy.outer * sy.chunks; sy.tw = P->tw[1].p; sy.kin_axis = nullptr; sy.kin_inner = nullptr;
-    launch_strided(Ny, 0, sy, cap, st);                                   // y forward
-    StridedArgs sx;
-    sx.data = HX; sx.ld = ldhx; sx.inner = (int64_t)Ny * Nz; sx.outer = 1; sx.chunks = (int)(sx.inner / 8);
-    sx.ntiles = (int64_t)nb * sx.chunks; sx.tw = P->tw[0].p; sx.kin_axis = P->kin_x.p; sx.kin_inner = P->kin_yz.p;
-    launch_strided(Nx, 2, sx, cap, st);                                   // x forward * t(k)/Ng, x inverse
-    launch_strided(Ny, 1, sy, cap, st);                                   // y inverse
-    launch_lines(Nz, 1, la, cap, st);                                     // z inverse + v(r) psi(r)
-    P->last_launches += 5;
+    Fft3Args fa;
+    fa.X = X; fa.W = HX; fa.HX = HX; fa.ldx = ldx; fa.ldw = ldhx; fa.ldhx = ldhx;
+    fa.ncol = nb; fa.nx = Nx; fa.ny = Ny; fa.nz = Nz; fa.my = Ny / 16;
+    fa.twx = P->tw[0].p; fa.twy = P->tw[1].p; fa.twz = P->tw[2].p;
+    fa.kin_x = P->kin_x.p; fa.kin_yz = P->kin_yz.p; fa.vloc = P->vloc.p;
+    RS_DISPATCH_N(Nz, launch_fwd_zy, fa, P->num_sms, st)                  // z fwd, y fwd stage A:  X -> HX
+    RS_CUDA(launch_x_any(Nx, fa, P->num_sms, st));                        // y B, x fwd, t(k)/Ng, x inv, y B'
+    RS_DISPATCH_N(Nz, launch_inv_yz, fa, P->num_sms, st)                  // y A', z inv, + v(r) psi(r)
+    P->last_launches += 3;
     if (nl) {
         for (size_t c = 0; c + 1 < P->colour_off.size(); ++c) {
             const int32_t *al = P->alist.p + P->colour_off[c];
