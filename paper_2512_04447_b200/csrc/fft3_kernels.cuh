@@ -46,8 +46,8 @@ __device__ __forceinline__ double2 ld_nc(const double2 *p) { return __ldg(p); }
 
 // ---------------------------------------------------------------------------------------------
 // z forward + y forward stage A.  128 threads; grid = G * my, CTA b works on n2y = b % my.
-template <int NZ>
-__global__ void __launch_bounds__(128, 4) fft3_fwd_zy_kernel(Fft3Args a)
+template <int NZ, int MINB>
+__global__ void __launch_bounds__(128, MINB) fft3_fwd_zy_kernel(Fft3Args a)
 {
     constexpr int MZ = NZ / 16;
     constexpr int RP = MZ * 17;                 // smem row pitch: 17 slots per 16-point group
@@ -113,8 +113,8 @@ __global__ void __launch_bounds__(128, 4) fft3_fwd_zy_kernel(Fft3Args a)
 // ---------------------------------------------------------------------------------------------
 // y inverse stage A' + z inverse + V_loc.  Mirror of the kernel above; W -> HX (may be in place:
 // a tile reads and writes the same 16 rows).
-template <int NZ>
-__global__ void __launch_bounds__(128, 4) fft3_inv_yz_kernel(Fft3Args a)
+template <int NZ, int MINB>
+__global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
 {
     constexpr int MZ = NZ / 16;
     constexpr int RP = MZ * 17;

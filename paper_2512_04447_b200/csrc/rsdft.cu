@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -89,10 +90,16 @@ struct rsdft_plan {
     DevBuf<int64_t> pt_off, beta_off;
     DevBuf<int32_t> idx, nproj_a;
     DevBuf<double> beta, Dmat;
-    std::vector<std::vector<int32_t>> colour_atoms;   // host copy of the colour classes
-    DevBuf<int32_t> alist;                            // concatenated colour classes
-    std::vector<int> colour_off;
-    DevBuf<double2> pq;                               // [natom][maxproj][batch]
+    int ncolour = 0, nchunks = 0;
+    std::vector<int> colour_chunk_off;                // chunks of colour c = [off[c], off[c+1])
+    DevBuf<rsdft::SphereChunk> chunks;                // sorted by (colour, atom, start)
+    DevBuf<int32_t> atom_chunk0, atom_chunks;         // per-atom chunk id lists
+    static constexpr int MAX_STREAMS = 4;
+    DevBuf<double2> pp[MAX_STREAMS];                  // [nchunks][maxproj][batch] partial projections
+    DevBuf<double2> pq[MAX_STREAMS];                  // [natom][maxproj][batch]   q = D p
+    int nstreams = 1;                                 // batches round-robin over internal streams
+    cudaStream_t s_batch[MAX_STREAMS] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[MAX_STREAMS] = {nullptr, nullptr, nullptr, nullptr};
 
     // apply_h batching
     int batch = 0;                // columns per kernel sequence
@@ -113,6 +120,11 @@ struct rsdft_plan {
     ~rsdft_plan()
     {
         for (auto e : ev) cudaEventDestroy(e);
+        for (int i = 0; i < MAX_STREAMS; ++i) {
+            if (s_batch[i]) cudaStreamDestroy(s_batch[i]);
+            if (ev_join[i]) cudaEventDestroy(ev_join[i]);
+        }
+        if (ev_fork) cudaEventDestroy(ev_fork);
         if (s_copy) cudaStreamDestroy(s_copy);
         if (s_comp) cudaStreamDestroy(s_comp);
     }
@@ -121,8 +133,9 @@ struct rsdft_plan {
         size_t b = 0;
         for (int a = 0; a < 3; ++a) b += tw[a].bytes();
         b += kin_x.bytes() + kin_yz.bytes() + vloc.bytes() + pt_off.bytes() + beta_off.bytes() + idx.bytes() +
-             nproj_a.bytes() + beta.bytes() + Dmat.bytes() + alist.bytes() + pq.bytes() + gram_work.bytes() +
-             gram_tiles.bytes() + hostY.bytes() + hostHY.bytes() + hostHS.bytes();
+             nproj_a.bytes() + beta.bytes() + Dmat.bytes() + chunks.bytes() + atom_chunk0.bytes() + atom_chunks.bytes() +
+             gram_work.bytes() + gram_tiles.bytes() + hostY.bytes() + hostHY.bytes() + hostHS.bytes();
+        for (int i = 0; i < MAX_STREAMS; ++i) b += pp[i].bytes() + pq[i].bytes();
         return b;
     }
 };
@@ -259,35 +272,46 @@ int build_spheres(rsdft_plan *P, const rsdft_atoms_t *atoms, const rsdft_project
     P->total_pts = pt_off[natom];
     P->max_pts = max_pts;
 
-    // colour classes: atoms whose spheres may share a grid point (|R_a - R_b|_min-image < rc_a + rc_b)
-    // get different colours; scatter-add then runs one launch per class without atomics.
-    std::vector<int> colour(natom, -1);
+    // colour classes: atoms of one colour have pairwise DISJOINT point sets (exact test on the
+    // index lists), so the scatter-add runs one launch per class without atomics.
+    std::vector<uint64_t> ptmask((size_t)P->ng, 0);
+    std::vector<int> colour(natom, 0);
     int ncolour = 0;
     for (int a = 0; a < natom; ++a) {
-        std::vector<char> used(ncolour + 1, 0);
-        for (int b = 0; b < a; ++b) {
-            double d2 = 0.0;
-            for (int ax = 0; ax < 3; ++ax) {
-                const double d = min_img(atoms->pos[3 * a + ax], atoms->pos[3 * b + ax], P->len[ax]);
-                d2 += d * d;
-            }
-            const double rr = proj->species[atoms->species[a]].rc + proj->species[atoms->species[b]].rc +
-                              (h[0] + h[1] + h[2]);
-            if (d2 < rr * rr) used[colour[b]] = 1;
-        }
+        uint64_t used = 0;
+        for (int64_t s = pt_off[a]; s < pt_off[a + 1]; ++s) used |= ptmask[idx[s]];
         int c = 0;
-        while (used[c]) ++c;
+        while (c < 64 && ((used >> c) & 1)) ++c;
+        if (c == 64) return fail(RSDFT_UNSUPPORTED, "rsdft_plan_create: more than 64 mutually overlapping projector spheres");
         colour[a] = c;
-        ncolour = std::max(ncolour, c + 1);
+        for (int64_t s = pt_off[a]; s < pt_off[a + 1]; ++s) ptmask[idx[s]] |= (uint64_t)1 << c;
+        if (pt_off[a + 1] > pt_off[a]) ncolour = std::max(ncolour, c + 1);
     }
-    P->colour_atoms.assign(ncolour, {});
-    for (int a = 0; a < natom; ++a) P->colour_atoms[colour[a]].push_back(a);
-    std::vector<int32_t> alist;
-    P->colour_off.assign(1, 0);
-    for (auto &v : P->colour_atoms) {
-        alist.insert(alist.end(), v.begin(), v.end());
-        P->colour_off.push_back((int)alist.size());
+    P->ncolour = ncolour;
+    // chunks of <= NL_PCH points, sorted by (colour, atom, start); per-atom chunk id lists
+    std::vector<rsdft::SphereChunk> chunks;
+    std::vector<std::vector<int32_t>> ids(natom);
+    P->colour_chunk_off.assign(1, 0);
+    for (int c = 0; c < ncolour; ++c) {
+        for (int a = 0; a < natom; ++a) {
+            if (colour[a] != c) continue;
+            const int64_t np = pt_off[a + 1] - pt_off[a];
+            for (int64_t st = 0; st < np; st += rsdft::NL_PCH) {
+                ids[a].push_back((int32_t)chunks.size());
+                chunks.push_back({a, (int32_t)st, (int32_t)std::min<int64_t>(rsdft::NL_PCH, np - st), 0});
+            }
+        }
+        P->colour_chunk_off.push_back((int)chunks.size());
     }
+    P->nchunks = (int)chunks.size();
+    std::vector<int32_t> atom_chunk0(natom + 1, 0), atom_chunks;
+    for (int a = 0; a < natom; ++a) {
+        atom_chunks.insert(atom_chunks.end(), ids[a].begin(), ids[a].end());
+        atom_chunk0[a + 1] = (int32_t)atom_chunks.size();
+    }
+    RS_CUDA(P->chunks.upload(chunks));
+    RS_CUDA(P->atom_chunk0.upload(atom_chunk0));
+    RS_CUDA(P->atom_chunks.upload(atom_chunks));
 
     RS_CUDA(P->pt_off.upload(pt_off));
     RS_CUDA(P->beta_off.upload(beta_off));
@@ -295,7 +319,6 @@ int build_spheres(rsdft_plan *P, const rsdft_atoms_t *atoms, const rsdft_project
     RS_CUDA(P->nproj_a.upload(nproj_a));
     RS_CUDA(P->beta.upload(beta));
     RS_CUDA(P->Dmat.upload(Dm));
-    RS_CUDA(P->alist.upload(alist));
     return RSDFT_OK;
 }
 
@@ -355,46 +378,60 @@ using namespace rsdft;
     default: break;                                                          \
     }
 
+int tune(const char *name, int dflt)
+{
+    const char *e = std::getenv(name);
+    return e ? atoi(e) : dflt;
+}
+
 // grid of the zy / yz kernels: G plane-walkers for each of the my row classes
-inline int rows_grid(const Fft3Args &a, int sms)
+inline int rows_grid(const Fft3Args &a, int sms, int occ)
 {
     const int64_t planes = (int64_t)a.ncol * a.nx;
-    const int64_t g = std::max<int64_t>(1, std::min<int64_t>(planes, (int64_t)sms * 8 / a.my));
+    const int64_t g = std::max<int64_t>(1, std::min<int64_t>(planes, (int64_t)sms * occ * 2 / a.my));
     return (int)(g * a.my);
 }
 
 template <int NZ>
 void launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    fft3_fwd_zy_kernel<NZ><<<rows_grid(a, sms), 128, 0, st>>>(a);
+    static const int occ = tune("RSDFT_ZY_OCC", 4);
+    if (occ >= 6) fft3_fwd_zy_kernel<NZ, 6><<<rows_grid(a, sms, 6), 128, 0, st>>>(a);
+    else if (occ == 5) fft3_fwd_zy_kernel<NZ, 5><<<rows_grid(a, sms, 5), 128, 0, st>>>(a);
+    else fft3_fwd_zy_kernel<NZ, 4><<<rows_grid(a, sms, 4), 128, 0, st>>>(a);
 }
 template <int NZ>
 void launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    fft3_inv_yz_kernel<NZ><<<rows_grid(a, sms), 128, 0, st>>>(a);
+    static const int occ = tune("RSDFT_YZ_OCC", 4);
+    if (occ >= 6) fft3_inv_yz_kernel<NZ, 6><<<rows_grid(a, sms, 6), 128, 0, st>>>(a);
+    else if (occ == 5) fft3_inv_yz_kernel<NZ, 5><<<rows_grid(a, sms, 5), 128, 0, st>>>(a);
+    else fft3_inv_yz_kernel<NZ, 4><<<rows_grid(a, sms, 4), 128, 0, st>>>(a);
 }
 
-constexpr int FFT3_TZ = 8;      // z points per x-kernel tile: 128 B contiguous per (x, row)
+template <int NX, int TZ, int NT, int MINB>
+cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    const size_t smem = (size_t)NX * (a.my * TZ + 1) * sizeof(double2);
+    const int64_t ntiles = (int64_t)a.ncol * 16 * (a.nz / TZ);
+    auto k = fft3_x_kernel<NX, TZ, NT, MINB>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int occ = (int)std::max<size_t>(1, std::min<size_t>(MINB, (227 * 1024) / (smem + 4096)));
+    k<<<(int)std::min<int64_t>(ntiles, (int64_t)sms * occ), NT, smem, st>>>(a);
+    return cudaSuccess;
+}
 
 template <int NX>
 cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    const size_t smem = (size_t)NX * (a.my * FFT3_TZ + 1) * sizeof(double2);
-    const int64_t ntiles = (int64_t)a.ncol * 16 * (a.nz / FFT3_TZ);
-    cudaError_t e;
-    if (2 * (smem + 4096) <= 227 * 1024) {
-        auto k = fft3_x_kernel<NX, FFT3_TZ, 256, 2>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        const int occ = (int)std::min<size_t>(2, (227 * 1024) / (smem + 4096));
-        k<<<(int)std::min<int64_t>(ntiles, (int64_t)sms * occ), 256, smem, st>>>(a);
-    } else {
-        auto k = fft3_x_kernel<NX, FFT3_TZ, 512, 1>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        k<<<(int)std::min<int64_t>(ntiles, sms), 512, smem, st>>>(a);
-    }
-    return cudaSuccess;
+    static const int cfg = tune("RSDFT_X_CFG", 0);
+    const size_t smem8 = (size_t)NX * (a.my * 8 + 1) * sizeof(double2);
+    if (cfg == 1) return launch_x_cfg<NX, 4, 256, 3>(a, sms, st);
+    if (cfg == 2) return launch_x_cfg<NX, 4, 128, 6>(a, sms, st);
+    if (cfg == 3) return launch_x_cfg<NX, 4, 128, 4>(a, sms, st);
+    if (2 * (smem8 + 4096) <= 227 * 1024) return launch_x_cfg<NX, 8, 256, 2>(a, sms, st);
+    return launch_x_cfg<NX, 8, 512, 1>(a, sms, st);
 }
 
 cudaError_t launch_x_any(int nx, const Fft3Args &a, int sms, cudaStream_t st)
@@ -415,16 +452,18 @@ cudaError_t launch_x_any(int nx, const Fft3Args &a, int sms, cudaStream_t st)
 }
 
 template <int NP>
-void launch_project_np(const SphereTables &t, const double2 *X, int64_t ldx, int ncol, double dV, double2 *p,
+void launch_project_np(const SphereTables &t, const double2 *X, int64_t ldx, int ncol, double dV, double2 *pp,
                        cudaStream_t st)
 {
-    project_kernel<NP><<<dim3(t.natom, ncol), 128, 0, st>>>(t, X, ldx, ncol, dV, p);
+    constexpr int CG = NlCols<NP>::CGP;
+    project_kernel<NP><<<dim3(t.nchunks, (ncol + CG - 1) / CG), NL_THREADS, 0, st>>>(t, X, ldx, ncol, dV, pp);
 }
 template <int NP>
-void launch_scatter_np(const SphereTables &t, const int32_t *alist, int nlist, const double2 *p, int ncol, double2 *HX,
+void launch_scatter_np(const SphereTables &t, int chunk0, int nlist, const double2 *q, int ncol, double2 *HX,
                        int64_t ldhx, cudaStream_t st)
 {
-    scatter_kernel<NP, false><<<dim3(nlist, ncol), 128, 0, st>>>(t, alist, p, ncol, HX, ldhx);
+    constexpr int CG = NlCols<NP>::CGS;
+    scatter_kernel<NP><<<dim3(nlist, (ncol + CG - 1) / CG), NL_THREADS, 0, st>>>(t, chunk0, q, ncol, HX, ldhx);
 }
 
 SphereTables sphere_tables(const rsdft_plan *P)
@@ -432,6 +471,7 @@ SphereTables sphere_tables(const rsdft_plan *P)
     SphereTables t;
     t.pt_off = P->pt_off.p; t.beta_off = P->beta_off.p; t.idx = P->idx.p; t.beta = P->beta.p;
     t.nproj = P->nproj_a.p; t.D = P->Dmat.p; t.natom = P->natom; t.maxproj = P->maxproj;
+    t.chunks = P->chunks.p; t.atom_chunk0 = P->atom_chunk0.p; t.atom_chunks = P->atom_chunks.p; t.nchunks = P->nchunks;
     return t;
 }
 
@@ -443,17 +483,19 @@ int default_batch(const rsdft_plan *P)
     return (int)std::max<int64_t>(1, std::min<int64_t>(b, 256));
 }
 
-// One batch of columns through the whole operator.
-int apply_h_batch(rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
+// One batch of columns through the whole operator, on stream slot `slot`.
+int apply_h_batch(rsdft_plan *P, int slot, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
 {
     const int Nx = P->n[0], Ny = P->n[1], Nz = P->n[2];
     const bool nl = P->natom > 0 && P->total_pts > 0;
     const SphereTables tabs = sphere_tables(P);
+    double2 *pp = P->pp[slot].p, *pq = P->pq[slot].p;
     if (nl) {   // projections read the INPUT orbitals
-        if (P->maxproj <= 4) launch_project_np<4>(tabs, X, ldx, nb, P->dV, P->pq.p, st);
-        else if (P->maxproj <= 9) launch_project_np<9>(tabs, X, ldx, nb, P->dV, P->pq.p, st);
-        else launch_project_np<16>(tabs, X, ldx, nb, P->dV, P->pq.p, st);
-        ++P->last_launches;
+        if (P->maxproj <= 4) launch_project_np<4>(tabs, X, ldx, nb, P->dV, pp, st);
+        else if (P->maxproj <= 9) launch_project_np<9>(tabs, X, ldx, nb, P->dV, pp, st);
+        else launch_project_np<16>(tabs, X, ldx, nb, P->dV, pp, st);
+        combine_kernel<<<dim3((nb + 127) / 128, P->natom), 128, 0, st>>>(tabs, pp, nb, pq);
+        P->last_launches += 2;
     }
     Fft3Args fa;
     fa.X = X; fa.W = HX; fa.HX = HX; fa.ldx = ldx; fa.ldw = ldhx; fa.ldhx = ldhx;
@@ -465,13 +507,12 @@ int apply_h_batch(rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 
     RS_DISPATCH_N(Nz, launch_inv_yz, fa, P->num_sms, st)                  // y A', z inv, + v(r) psi(r)
     P->last_launches += 3;
     if (nl) {
-        for (size_t c = 0; c + 1 < P->colour_off.size(); ++c) {
-            const int32_t *al = P->alist.p + P->colour_off[c];
-            const int nlist = P->colour_off[c + 1] - P->colour_off[c];
+        for (int c = 0; c < P->ncolour; ++c) {
+            const int ch0 = P->colour_chunk_off[c], nlist = P->colour_chunk_off[c + 1] - ch0;
             if (nlist == 0) continue;
-            if (P->maxproj <= 4) launch_scatter_np<4>(tabs, al, nlist, P->pq.p, nb, HX, ldhx, st);
-            else if (P->maxproj <= 9) launch_scatter_np<9>(tabs, al, nlist, P->pq.p, nb, HX, ldhx, st);
-            else launch_scatter_np<16>(tabs, al, nlist, P->pq.p, nb, HX, ldhx, st);
+            if (P->maxproj <= 4) launch_scatter_np<4>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
+            else if (P->maxproj <= 9) launch_scatter_np<9>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
+            else launch_scatter_np<16>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
             ++P->last_launches;
         }
     }
@@ -483,12 +524,35 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
 {
     const int batch = P->user_batch > 0 ? P->user_batch : default_batch(P);
     P->batch = batch;
-    if (P->natom > 0) RS_CUDA(P->pq.ensure((size_t)P->natom * P->maxproj * batch));
-    for (int c0 = 0; c0 < ncol; c0 += batch) {
+    const int nbatches = (ncol + batch - 1) / batch;
+    const int ns = std::max(1, std::min(std::min(P->nstreams, (int)rsdft_plan::MAX_STREAMS), nbatches));
+    if (P->natom > 0 && P->total_pts > 0)
+        for (int i = 0; i < ns; ++i) {
+            RS_CUDA(P->pp[i].ensure((size_t)P->nchunks * P->maxproj * batch));
+            RS_CUDA(P->pq[i].ensure((size_t)P->natom * P->maxproj * batch));
+        }
+    if (ns > 1) {   // fork: the internal streams start after everything already queued on `st`
+        if (!P->ev_fork) RS_CUDA(cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming));
+        for (int i = 0; i < ns; ++i) {
+            if (!P->s_batch[i]) RS_CUDA(cudaStreamCreateWithFlags(&P->s_batch[i], cudaStreamNonBlocking));
+            if (!P->ev_join[i]) RS_CUDA(cudaEventCreateWithFlags(&P->ev_join[i], cudaEventDisableTiming));
+        }
+        RS_CUDA(cudaEventRecord(P->ev_fork, st));
+        for (int i = 0; i < ns; ++i) RS_CUDA(cudaStreamWaitEvent(P->s_batch[i], P->ev_fork, 0));
+    }
+    int k = 0;
+    for (int c0 = 0; c0 < ncol; c0 += batch, ++k) {
         const int nb = std::min(batch, ncol - c0);
-        const int rc = apply_h_batch(P, nb, X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx, st);
+        const int slot = ns > 1 ? k % ns : 0;
+        const int rc = apply_h_batch(P, slot, nb, X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx,
+                                     ns > 1 ? P->s_batch[slot] : st);
         if (rc != RSDFT_OK) return rc;
     }
+    if (ns > 1)     // join
+        for (int i = 0; i < ns; ++i) {
+            RS_CUDA(cudaEventRecord(P->ev_join[i], P->s_batch[i]));
+            RS_CUDA(cudaStreamWaitEvent(st, P->ev_join[i], 0));
+        }
     return RSDFT_OK;
 }
 
@@ -609,6 +673,7 @@ int rsdft_plan_create(const rsdft_grid_t *grid, const rsdft_box_t *box, const rs
         rc = fail(RSDFT_ALLOC, "rsdft_plan_create: host allocation failed");
     }
     if (rc != RSDFT_OK) { delete P; return rc; }
+    if (const char *e = std::getenv("RSDFT_STREAMS")) P->nstreams = std::max(1, std::min(atoi(e), (int)rsdft_plan::MAX_STREAMS));
     *out = P;
     return RSDFT_OK;
 }
@@ -642,7 +707,7 @@ int rsdft_plan_info(const rsdft_plan_t *plan, int64_t *out8)
     if (!plan || !out8) return fail(RSDFT_INVALID_ARG, "rsdft_plan_info: null argument");
     out8[0] = plan->natom; out8[1] = plan->total_pts; out8[2] = plan->max_pts; out8[3] = (int64_t)plan->device_bytes();
     out8[4] = plan->user_batch > 0 ? plan->user_batch : default_batch(plan); out8[5] = plan->last_launches;
-    out8[6] = plan->ng; out8[7] = (int64_t)plan->colour_atoms.size();
+    out8[6] = plan->ng; out8[7] = plan->ncolour;
     return RSDFT_OK;
 }
 
