@@ -229,7 +229,7 @@ def run_ours(args):
     peaks = probe_peaks() if rank == 0 else None
 
     # Y = [X, W, P] resident in HBM (seeded per column; every rank draws the same block)
-    Y = torch.cat([wl.orbital_block(ng, range(m), system["seed"], s, device="cuda") for s in range(3)], dim=0)
+    Y = wl.block_y(system, device="cuda")
     HY = torch.empty_like(Y)
     Hs = torch.empty((n, n), dtype=torch.complex128, device="cuda")
     Ss = torch.empty((n, n), dtype=torch.complex128, device="cuda")

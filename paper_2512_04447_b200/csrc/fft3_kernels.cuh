@@ -25,6 +25,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include "async_copy.cuh"
 #include "fft_codelets.cuh"
 
 namespace rsdft {
@@ -45,6 +46,15 @@ struct Fft3Args {
 __device__ __forceinline__ double2 ld_nc(const double2 *p) { return __ldg(p); }
 
 // ---------------------------------------------------------------------------------------------
+// shared-memory geometry of the 16-row tiles of the zy / yz kernels
+template <int NZ>
+struct ZyCfg {
+    static constexpr int MZ = NZ / 16;
+    static constexpr int RP = MZ * 17;                 // smem row pitch: 17 slots per 16-point group
+    static constexpr int TILE = 16 * RP;               // double2 elements per tile buffer
+    static constexpr size_t SMEM_INV = (size_t)(2 * TILE + 16 * NZ) * sizeof(double2);
+};
+
 // z forward + y forward stage A.  128 threads; grid = G * my, CTA b works on n2y = b % my.
 template <int NZ, int MINB>
 __global__ void __launch_bounds__(128, MINB) fft3_fwd_zy_kernel(Fft3Args a)
@@ -112,14 +122,17 @@ __global__ void __launch_bounds__(128, MINB) fft3_fwd_zy_kernel(Fft3Args a)
 
 // ---------------------------------------------------------------------------------------------
 // y inverse stage A' + z inverse + V_loc.  Mirror of the kernel above; W -> HX (may be in place:
-// a tile reads and writes the same 16 rows).
-template <int NZ, int MINB>
-__global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
+// a tile reads and writes the same 16 rows).  CTA b owns n2y = b % my and the x planes
+// g0, g0 + G, ...; for each plane it runs over ALL columns of the batch (the 16 rows of v(r) stay
+// hot in L1/L2).  Per tile: the k-space rows of the NEXT tile (double buffered) and the psi rows of
+// THIS tile (consumed two phases later) arrive by cp.async.
+template <int NZ>
+__global__ void __launch_bounds__(128, 2) fft3_inv_yz_kernel(Fft3Args a)
 {
-    constexpr int MZ = NZ / 16;
-    constexpr int RP = MZ * 17;
-    constexpr int NT = 128;
-    __shared__ double2 S[16 * RP];
+    constexpr int MZ = ZyCfg<NZ>::MZ, RP = ZyCfg<NZ>::RP, TILE = ZyCfg<NZ>::TILE, NT = 128;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2 *Sw0 = reinterpret_cast<double2 *>(smem_raw);
+    double2 *Sp = Sw0 + 2 * TILE;                               // psi rows, dense [16][NZ]
     __shared__ double2 twz_s[(MZ > 1 ? MZ - 1 : 1) * 16];
     __shared__ double2 twy_s[16];
     const int tid = threadIdx.x;
@@ -128,26 +141,60 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
     const int g0 = blockIdx.x / my, G = gridDim.x / my;
     for (int e = tid; e < (MZ - 1) * 16; e += NT) twz_s[e] = a.twz[(e & 15) * ((e >> 4) + 1)];
     if (tid < 16) twy_s[tid] = a.twy[n2y * tid];
-    __syncthreads();
-    const int64_t nplanes = (int64_t)a.ncol * a.nx;
-    for (int64_t cx = g0; cx < nplanes; cx += G) {
-        const int64_t col = cx / a.nx;
-        const int64_t x = cx - col * a.nx;
-        const double2 *src = a.W + col * a.ldw + x * a.ny * NZ;
-        const double2 *psi = a.X + col * a.ldx + x * a.ny * NZ;
-        const double *vl = a.vloc + x * a.ny * NZ;
-        double2 *dst = a.HX + col * a.ldhx + x * a.ny * NZ;
-        // y inverse stage A': conj twiddle, radix-16 over k1y (swapped domain) -> row j = n1y
+    const int nxm = g0 < a.nx ? (a.nx - g0 + G - 1) / G : 0;      // planes of this walker
+    const int64_t T = (int64_t)nxm * a.ncol;                      // tiles: plane-major, column-minor
+    auto plane_off = [&](int64_t t, int64_t &col) -> int64_t {
+        const int64_t i = t / a.ncol;
+        col = t - i * a.ncol;
+        return (g0 + i * G) * (int64_t)a.ny * NZ;
+    };
+    auto issue_w = [&](int buf, int64_t t) {
+        int64_t col;
+        const int64_t po = plane_off(t, col);
+        const double2 *src = a.W + col * a.ldw + po;
+        double2 *S = Sw0 + buf * TILE;
+#pragma unroll
+        for (int e = tid; e < 16 * NZ; e += NT) {
+            const int k = e / NZ, p = e - k * NZ;
+            cp_async16(S + k * RP + (p >> 4) * 17 + (p & 15), src + (int64_t)(k * my + n2y) * NZ + p);
+        }
+    };
+    auto issue_psi = [&](int64_t t) {
+        int64_t col;
+        const int64_t po = plane_off(t, col);
+        const double2 *src = a.X + col * a.ldx + po;
+#pragma unroll
+        for (int e = tid; e < 16 * NZ; e += NT) {
+            const int j = e / NZ, p = e - j * NZ;
+            cp_async16(Sp + e, src + (int64_t)(j * my + n2y) * NZ + p);
+        }
+    };
+    if (T > 0) issue_w(0, 0);
+    cp_async_commit();
+    int buf = 0;
+    for (int64_t t = 0; t < T; ++t, buf ^= 1) {
+        issue_psi(t);
+        cp_async_commit();
+        if (t + 1 < T) issue_w(buf ^ 1, t + 1);
+        cp_async_commit();
+        cp_async_wait<2>();                                       // W(t) has landed
+        __syncthreads();
+        int64_t col;
+        const int64_t po = plane_off(t, col);
+        double2 *S = Sw0 + buf * TILE;
+        const double *vl = a.vloc + po;
+        double2 *dst = a.HX + col * a.ldhx + po;
+        // y inverse stage A': conj twiddle, radix-16 over k1y (swapped domain) -> row j = n1y, in place
         for (int p = tid; p < NZ; p += NT) {
-            const int sp = (p >> 4) * 17 + (p & 15);
+            double2 *c = S + (p >> 4) * 17 + (p & 15);
             double br[16], bi[16];
 #pragma unroll
-            for (int k = 0; k < 16; ++k) { const double2 v = src[(int64_t)(k * my + n2y) * NZ + p]; br[k] = v.x; bi[k] = v.y; }
+            for (int k = 0; k < 16; ++k) { const double2 v = c[k * RP]; br[k] = v.x; bi[k] = v.y; }
 #pragma unroll
             for (int k = 1; k < 16; ++k) { const double2 w = twy_s[k]; tw_mul(bi[k], br[k], w.x, -w.y); }
             Dft<16>::run(bi, br);
 #pragma unroll
-            for (int j = 0; j < 16; ++j) S[j * RP + sp] = make_double2(br[j], bi[j]);
+            for (int j = 0; j < 16; ++j) c[j * RP] = make_double2(br[j], bi[j]);
         }
         __syncthreads();
         // z inverse stage B': radix-16 over k2z (swapped), in place
@@ -155,11 +202,12 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
             double2 *p = S + item * 17;
             double br[16], bi[16];
 #pragma unroll
-            for (int t = 0; t < 16; ++t) { const double2 v = p[t]; br[t] = v.x; bi[t] = v.y; }
+            for (int q = 0; q < 16; ++q) { const double2 v = p[q]; br[q] = v.x; bi[q] = v.y; }
             Dft<16>::run(bi, br);
 #pragma unroll
-            for (int t = 0; t < 16; ++t) p[t] = make_double2(br[t], bi[t]);
+            for (int q = 0; q < 16; ++q) p[q] = make_double2(br[q], bi[q]);
         }
+        cp_async_wait<1>();                                       // psi(t) has landed
         __syncthreads();
         // z inverse stage A': conj twiddle, radix-MZ over k1z (swapped) -> z = n1*16 + n2; + v psi
 #pragma unroll
@@ -174,13 +222,14 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
             const int64_t off = (int64_t)(j * my + n2y) * NZ + n2;
 #pragma unroll
             for (int n1 = 0; n1 < MZ; ++n1) {
-                const double2 ps = ld_nc(psi + off + n1 * 16);
+                const double2 ps = Sp[j * NZ + n1 * 16 + n2];
                 const double vv = __ldg(vl + off + n1 * 16);
                 dst[off + n1 * 16] = make_double2(fma(vv, ps.x, re[n1]), fma(vv, ps.y, im[n1]));
             }
         }
         __syncthreads();
     }
+    cp_async_wait<0>();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -189,7 +238,25 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
 template <int MY, int NX, int TZ, int NT>
 __device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *base, double2 *S, int P, int tid)
 {
-    for (int item = tid; item < NX * TZ; item += NT) {
+    // items are taken two at a time so that both items' global loads are in flight together
+    int item = tid;
+    for (; item + NT < NX * TZ; item += 2 * NT) {
+        const int z0 = item % TZ, x0 = item / TZ, z1 = (item + NT) % TZ, x1 = (item + NT) / TZ;
+        const double2 *p0 = base + (int64_t)x0 * a.ny * a.nz + z0;
+        const double2 *p1 = base + (int64_t)x1 * a.ny * a.nz + z1;
+        double re0[MY], im0[MY], re1[MY], im1[MY];
+#pragma unroll
+        for (int j = 0; j < MY; ++j) { const double2 v = p0[(int64_t)j * a.nz]; re0[j] = v.x; im0[j] = v.y; }
+#pragma unroll
+        for (int j = 0; j < MY; ++j) { const double2 v = p1[(int64_t)j * a.nz]; re1[j] = v.x; im1[j] = v.y; }
+        Dft<MY>::run(re0, im0);
+#pragma unroll
+        for (int j = 0; j < MY; ++j) S[x0 * P + j * TZ + z0] = make_double2(re0[j], im0[j]);
+        Dft<MY>::run(re1, im1);
+#pragma unroll
+        for (int j = 0; j < MY; ++j) S[x1 * P + j * TZ + z1] = make_double2(re1[j], im1[j]);
+    }
+    if (item < NX * TZ) {
         const int z = item % TZ, x = item / TZ;
         const double2 *ptr = base + (int64_t)x * a.ny * a.nz + z;
         double re[MY], im[MY];
@@ -216,8 +283,20 @@ __device__ __forceinline__ void fft3_x_store_y(const Fft3Args &a, double2 *base,
     }
 }
 
+// Per-length launch shape: z points per tile (TZ*16 B contiguous per row), threads, CTAs per SM.
+// (NT = 288 for 96, which fills the radix-16 phase in one round, measured 40 % slower than 256.)
+template <int NX> struct XCfg;
+template <> struct XCfg<16> { static constexpr int TZ = 8, NT = 32, MINB = 8; };
+template <> struct XCfg<32> { static constexpr int TZ = 8, NT = 64, MINB = 8; };
+template <> struct XCfg<48> { static constexpr int TZ = 8, NT = 96, MINB = 5; };
+template <> struct XCfg<64> { static constexpr int TZ = 8, NT = 128, MINB = 4; };
+template <> struct XCfg<80> { static constexpr int TZ = 8, NT = 224, MINB = 2; };
+template <> struct XCfg<96> { static constexpr int TZ = 8, NT = 256, MINB = 2; };
+template <> struct XCfg<112> { static constexpr int TZ = 8, NT = 256, MINB = 2; };
+template <> struct XCfg<128> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
+
 template <int NX, int TZ, int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) fft3_x_kernel(Fft3Args a)
+__global__ void __maxnreg__(((65536 / (NT * MINB)) / 8 * 8) > 255 ? 255 : ((65536 / (NT * MINB)) / 8 * 8)) fft3_x_kernel(Fft3Args a)
 {
     constexpr int MX = NX / 16;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -233,8 +312,9 @@ __global__ void __launch_bounds__(NT, MINB) fft3_x_kernel(Fft3Args a)
     const int64_t per_col = (int64_t)16 * zchunks;
     const int64_t ntiles = per_col * a.ncol;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int64_t col = tile / per_col;
-        const int rem = (int)(tile - col * per_col);
+        const int64_t colf = tile / per_col;
+        const int rem = (int)(tile - colf * per_col);
+        const int64_t col = a.ncol - 1 - colf;     // zig-zag: the forward kernel ended on the last column, start there (L2)
         const int k1y = rem / zchunks, zc = rem - k1y * zchunks;
         double2 *base = a.W + col * a.ldw + (int64_t)(k1y * my) * a.nz + zc * TZ;
         switch (my) {

@@ -17,6 +17,7 @@
 // workspace; gram_reduce_kernel then sums the slabs in a fixed order (deterministic), mirrors
 // S_sub and writes both triangles.
 #pragma once
+#include "async_copy.cuh"
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -40,14 +41,6 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
-
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
-{
-    const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
 // CTA tile (WGM*FA*8) x (WGN*FB*8) complex outputs, WGM*WGN warps, each warp FA x FB DMMA tiles.
 // KC grid points per pipeline stage, smem row pitch KC+4 complex (pitch % 8 == 4 -> the 8 lanes

@@ -3,9 +3,9 @@
 //   project:  pp[k][i][c] = dV * sum_{s in chunk k} beta[a][i][s] * psi_c(idx[a][s])
 //   combine:  q[a][i][c]  = sum_j D_a[i][j] * sum_{k in chunks(a)} pp[k][j][c]      (fixed order)
 //   scatter:  HX_c(idx[a][s]) += sum_i beta[a][i][s] * q[a][i][c]
-// Every sphere is cut into chunks of <= PCH points; one CTA owns (chunk, group of CG columns):
-// idx and beta are read ONCE per point and reused for the CG columns, whose gathers are
-// independent loads in flight.  Partial projections are combined in a fixed order, and the
+// Every sphere is cut into chunks of <= PCH points; idx and beta are read ONCE per (chunk, column
+// group) and reused for the group's columns, whose gathers are independent loads in flight.
+// Partial projections are combined in a fixed order, and the
 // scatter runs one launch per colour class (spheres of a class are pairwise disjoint), so the
 // result is deterministic and bitwise independent of the column batching.
 #pragma once
@@ -14,7 +14,13 @@
 
 namespace rsdft {
 
-constexpr int NL_PCH = 256;       // sphere points per chunk
+__device__ __forceinline__ void nl_dmma884(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+constexpr int NL_PCH = 128;       // sphere points per chunk
 constexpr int NL_THREADS = 128;
 
 struct SphereChunk {
@@ -37,99 +43,132 @@ struct SphereTables {
     int32_t natom, maxproj, nchunks;
 };
 
-// columns per CTA.  project: NP*CG complex accumulators (4 registers each) stay <= 72 registers;
 // scatter: CG complex values in flight per point.
 template <int NP> struct NlCols {
-    static constexpr int CGP = NP <= 4 ? 4 : (NP <= 9 ? 2 : 1);
     static constexpr int CGS = NP <= 4 ? 8 : (NP <= 9 ? 4 : 2);
 };
 
-template <int NP>
-__global__ void __launch_bounds__(NL_THREADS) project_kernel(SphereTables t, const double2 *__restrict__ X, int64_t ldx,
-                                                             int32_t ncol, double dV, double2 *__restrict__ pp)
+// Projection as a skinny FP64 tensor-core contraction with a gathered operand:
+//   P[i][c] = sum_s beta[i][s] * psi_c(idx[s]),   M = projectors (MT tiles of 8), K = sphere points,
+//   N = columns; real and imaginary parts of 8 columns are two N-tiles fed by ONE 16-byte gather.
+// One warp owns (chunk, 8*G8 columns): beta and idx are read once per chunk and reused for all its
+// columns, partial sums live in DMMA accumulators (no cross-lane reduction), and 8 k-steps of gathers
+// are in flight per lane.  mma.m8n8k4 fragments: A[row = lane/4][k = lane%4], B[k = lane%4][col = lane/4],
+// D[row = lane/4][col = 2*(lane%4) + {0, 1}].
+template <int MT, int G8>
+__global__ void __launch_bounds__(128) project_kernel(SphereTables t, const double2 *__restrict__ X, int64_t ldx,
+                                                      int32_t ncol, double dV, double2 *__restrict__ pp)
 {
-    constexpr int CG = NlCols<NP>::CGP;
-    const SphereChunk ch = t.chunks[blockIdx.x];
-    const int c0 = blockIdx.y * CG;
+    const int lane = threadIdx.x & 31;
+    const int chunk_id = blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (chunk_id >= t.nchunks) return;                       // warp-uniform; the kernel has no block barrier
+    const SphereChunk ch = t.chunks[chunk_id];
+    const int c0 = (gridDim.y - 1 - blockIdx.y) * 8 * G8;   // last columns first: the FFT that follows starts on column 0 (L2)
     const int a = ch.atom;
     const int64_t o = t.pt_off[a];
     const int npts = (int)(t.pt_off[a + 1] - o);
     const int np = t.nproj[a];
     const int32_t *idx = t.idx + o + ch.start;
     const double *beta = t.beta + t.beta_off[a] + ch.start;
-    const double2 *psi = X + (int64_t)c0 * ldx;
-    const int nc = min(CG, ncol - c0);
-    double ar[NP][CG], ai[NP][CG];
+    const int kq = lane & 3, r8 = lane >> 2;
+    const double2 *colp[G8];
+    bool colok[G8];
 #pragma unroll
-    for (int i = 0; i < NP; ++i)
+    for (int g = 0; g < G8; ++g) {
+        const int c = c0 + g * 8 + r8;
+        colok[g] = c < ncol;
+        colp[g] = X + (int64_t)(colok[g] ? c : 0) * ldx;
+    }
+    const double *brow[MT];
+    bool rowok[MT];
 #pragma unroll
-        for (int c = 0; c < CG; ++c) { ar[i][c] = 0.0; ai[i][c] = 0.0; }
-    for (int s = threadIdx.x; s < ch.count; s += NL_THREADS) {
-        const int64_t g = idx[s];
-        double2 v[CG];
+    for (int m = 0; m < MT; ++m) {
+        const int i = m * 8 + r8;
+        rowok[m] = i < np;
+        brow[m] = beta + (int64_t)(rowok[m] ? i : 0) * npts;
+    }
+    double are[MT][G8][2], aim[MT][G8][2];
 #pragma unroll
-        for (int c = 0; c < CG; ++c) v[c] = c < nc ? __ldg(psi + (int64_t)c * ldx + g) : make_double2(0.0, 0.0);
+    for (int m = 0; m < MT; ++m)
 #pragma unroll
-        for (int i = 0; i < NP; ++i) {
-            const double b = i < np ? __ldg(beta + (int64_t)i * npts + s) : 0.0;
+        for (int g = 0; g < G8; ++g) { are[m][g][0] = are[m][g][1] = aim[m][g][0] = aim[m][g][1] = 0.0; }
+    for (int s0 = 0; s0 < ch.count; s0 += 32) {
+        const int32_t my_idx = idx[min(s0 + lane, ch.count - 1)];            // one coalesced read per 8 k-steps
 #pragma unroll
-            for (int c = 0; c < CG; ++c) {
-                ar[i][c] = fma(b, v[c].x, ar[i][c]);
-                ai[i][c] = fma(b, v[c].y, ai[i][c]);
+        for (int j = 0; j < 8; ++j) {
+            const int s = s0 + 4 * j + kq;
+            const bool ok = s < ch.count;                                     // past the end: beta = 0 on a valid address
+            const int64_t g = __shfl_sync(0xffffffffu, my_idx, 4 * j + kq);
+            double av[MT];
+#pragma unroll
+            for (int m = 0; m < MT; ++m) av[m] = (ok && rowok[m]) ? __ldg(brow[m] + s) : 0.0;
+#pragma unroll
+            for (int gg = 0; gg < G8; ++gg) {
+                const double2 v = colok[gg] ? __ldg(colp[gg] + g) : make_double2(0.0, 0.0);
+#pragma unroll
+                for (int m = 0; m < MT; ++m) {
+                    nl_dmma884(are[m][gg][0], are[m][gg][1], av[m], v.x);
+                    nl_dmma884(aim[m][gg][0], aim[m][gg][1], av[m], v.y);
+                }
             }
         }
     }
-    __shared__ double red[NL_THREADS / 32][NP][CG][2];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
 #pragma unroll
-    for (int i = 0; i < NP; ++i)
+    for (int m = 0; m < MT; ++m) {
+        const int i = m * 8 + r8;
+        if (i >= np) continue;
 #pragma unroll
-        for (int c = 0; c < CG; ++c) {
-            double r = ar[i][c], m = ai[i][c];
+        for (int g = 0; g < G8; ++g)
 #pragma unroll
-            for (int sft = 16; sft > 0; sft >>= 1) {
-                r += __shfl_xor_sync(0xffffffffu, r, sft);
-                m += __shfl_xor_sync(0xffffffffu, m, sft);
+            for (int e = 0; e < 2; ++e) {
+                const int c = c0 + g * 8 + 2 * kq + e;
+                if (c < ncol) pp[((int64_t)chunk_id * t.maxproj + i) * ncol + c] = make_double2(dV * are[m][g][e], dV * aim[m][g][e]);
             }
-            if (lane == 0) { red[w][i][c][0] = r; red[w][i][c][1] = m; }
-        }
-    __syncthreads();
-    for (int e = threadIdx.x; e < NP * CG; e += NL_THREADS) {
-        const int i = e / CG, c = e - i * CG;
-        if (i < np && c < nc) {
-            const double sr = (red[0][i][c][0] + red[1][i][c][0]) + (red[2][i][c][0] + red[3][i][c][0]);
-            const double si = (red[0][i][c][1] + red[1][i][c][1]) + (red[2][i][c][1] + red[3][i][c][1]);
-            pp[((int64_t)blockIdx.x * t.maxproj + i) * ncol + c0 + c] = make_double2(dV * sr, dV * si);
-        }
     }
 }
 
-// q[a][i][c] = sum_j D_a[i][j] * (sum over the atom's chunks, ascending start, of pp[k][j][c])
+// q[a][i][c] = sum_j D_a[i][j] * (sum over the atom's chunks, ascending start, of pp[k][j][c]).
+// One CTA per (atom, tile of NL_CCOLS columns): every thread sums the chunk partials of one (j, c)
+// pair (independent loads, fixed order), then one (i, c) row of D.
+constexpr int NL_CCOLS = 32;
 __global__ void __launch_bounds__(128) combine_kernel(SphereTables t, const double2 *__restrict__ pp, int32_t ncol,
                                                       double2 *__restrict__ q)
 {
-    const int a = blockIdx.y;
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncol) return;
+    const int a = blockIdx.x;
+    const int c0 = blockIdx.y * NL_CCOLS;
+    const int nc = min(NL_CCOLS, ncol - c0);
     const int np = t.nproj[a], mp = t.maxproj;
     const int k0 = t.atom_chunk0[a], k1 = t.atom_chunk0[a + 1];
-    double pr[16], pi[16];
-    for (int j = 0; j < np; ++j) {
+    __shared__ double2 ps[16][NL_CCOLS];
+    for (int e = threadIdx.x; e < np * nc; e += blockDim.x) {
+        const int j = e / nc, c = e - j * nc;
+        const double2 *src = pp + (int64_t)j * ncol + c0 + c;
         double sr = 0.0, si = 0.0;
-        for (int k = k0; k < k1; ++k) {
-            const double2 v = pp[((int64_t)t.atom_chunks[k] * mp + j) * ncol + c];
+        int k = k0;
+        for (; k + 4 <= k1; k += 4) {
+            double2 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[u] = src[(int64_t)t.atom_chunks[k + u] * mp * ncol];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { sr += v[u].x; si += v[u].y; }
+        }
+        for (; k < k1; ++k) {
+            const double2 v = src[(int64_t)t.atom_chunks[k] * mp * ncol];
             sr += v.x; si += v.y;
         }
-        pr[j] = sr; pi[j] = si;
+        ps[j][c] = make_double2(sr, si);
     }
+    __syncthreads();
     const double *D = t.D + (int64_t)a * mp * mp;
-    for (int i = 0; i < np; ++i) {
+    for (int e = threadIdx.x; e < np * nc; e += blockDim.x) {
+        const int i = e / nc, c = e - i * nc;
         double sr = 0.0, si = 0.0;
         for (int j = 0; j < np; ++j) {
-            sr = fma(D[i * np + j], pr[j], sr);
-            si = fma(D[i * np + j], pi[j], si);
+            const double d = D[i * np + j];
+            sr = fma(d, ps[j][c].x, sr);
+            si = fma(d, ps[j][c].y, si);
         }
-        q[((int64_t)a * mp + i) * ncol + c] = make_double2(sr, si);
+        q[((int64_t)a * mp + i) * ncol + c0 + c] = make_double2(sr, si);
     }
 }
 
@@ -141,7 +180,7 @@ __global__ void __launch_bounds__(NL_THREADS) scatter_kernel(SphereTables t, int
     // read-modify-write below is race-free and the result is deterministic)
     constexpr int CG = NlCols<NP>::CGS;
     const SphereChunk ch = t.chunks[chunk0 + blockIdx.x];
-    const int c0 = blockIdx.y * CG;
+    const int c0 = (gridDim.y - 1 - blockIdx.y) * CG;   // last columns first: the FFT before ended there (L2)
     const int a = ch.atom;
     const int64_t o = t.pt_off[a];
     const int npts = (int)(t.pt_off[a + 1] - o);

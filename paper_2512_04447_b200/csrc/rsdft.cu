@@ -97,7 +97,7 @@ struct rsdft_plan {
     static constexpr int MAX_STREAMS = 4;
     DevBuf<double2> pp[MAX_STREAMS];                  // [nchunks][maxproj][batch] partial projections
     DevBuf<double2> pq[MAX_STREAMS];                  // [natom][maxproj][batch]   q = D p
-    int nstreams = 1;                                 // batches round-robin over internal streams
+    int nstreams = 3;                                 // batches round-robin over internal streams (RSDFT_STREAMS overrides)
     cudaStream_t s_batch[MAX_STREAMS] = {nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[MAX_STREAMS] = {nullptr, nullptr, nullptr, nullptr};
 
@@ -365,17 +365,17 @@ namespace {
 
 using namespace rsdft;
 
-#define RS_DISPATCH_N(N_, FN_, ...)                                          \
+#define RS_DISPATCH_N(ERR_, N_, FN_, ...)                                    \
     switch (N_) {                                                            \
-    case 16: FN_<16>(__VA_ARGS__); break;                                    \
-    case 32: FN_<32>(__VA_ARGS__); break;                                    \
-    case 48: FN_<48>(__VA_ARGS__); break;                                    \
-    case 64: FN_<64>(__VA_ARGS__); break;                                    \
-    case 80: FN_<80>(__VA_ARGS__); break;                                    \
-    case 96: FN_<96>(__VA_ARGS__); break;                                    \
-    case 112: FN_<112>(__VA_ARGS__); break;                                  \
-    case 128: FN_<128>(__VA_ARGS__); break;                                  \
-    default: break;                                                          \
+    case 16: ERR_ = FN_<16>(__VA_ARGS__); break;                             \
+    case 32: ERR_ = FN_<32>(__VA_ARGS__); break;                             \
+    case 48: ERR_ = FN_<48>(__VA_ARGS__); break;                             \
+    case 64: ERR_ = FN_<64>(__VA_ARGS__); break;                             \
+    case 80: ERR_ = FN_<80>(__VA_ARGS__); break;                             \
+    case 96: ERR_ = FN_<96>(__VA_ARGS__); break;                             \
+    case 112: ERR_ = FN_<112>(__VA_ARGS__); break;                           \
+    case 128: ERR_ = FN_<128>(__VA_ARGS__); break;                           \
+    default: ERR_ = cudaErrorInvalidValue; break;                            \
     }
 
 int tune(const char *name, int dflt)
@@ -384,40 +384,46 @@ int tune(const char *name, int dflt)
     return e ? atoi(e) : dflt;
 }
 
-// grid of the zy / yz kernels: G plane-walkers for each of the my row classes
-inline int rows_grid(const Fft3Args &a, int sms, int occ)
+// CTAs per SM that fit by shared memory (1 KB reserved per CTA), capped
+inline int occ_by_smem(size_t smem, int cap)
 {
-    const int64_t planes = (int64_t)a.ncol * a.nx;
-    const int64_t g = std::max<int64_t>(1, std::min<int64_t>(planes, (int64_t)sms * occ * 2 / a.my));
-    return (int)(g * a.my);
+    return (int)std::max<size_t>(1, std::min<size_t>((size_t)cap, (size_t)(228 * 1024) / (smem + 2048)));
 }
 
 template <int NZ>
-void launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
+cudaError_t launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    static const int occ = tune("RSDFT_ZY_OCC", 4);
-    if (occ >= 6) fft3_fwd_zy_kernel<NZ, 6><<<rows_grid(a, sms, 6), 128, 0, st>>>(a);
-    else if (occ == 5) fft3_fwd_zy_kernel<NZ, 5><<<rows_grid(a, sms, 5), 128, 0, st>>>(a);
-    else fft3_fwd_zy_kernel<NZ, 4><<<rows_grid(a, sms, 4), 128, 0, st>>>(a);
+    // G plane-walkers for each of the my row classes, two CTA generations of 4 per SM
+    const int64_t planes = (int64_t)a.ncol * a.nx;
+    const int64_t g = std::max<int64_t>(1, std::min<int64_t>(planes, (int64_t)sms * 8 / a.my));
+    fft3_fwd_zy_kernel<NZ, 4><<<(int)(g * a.my), 128, 0, st>>>(a);
+    return cudaSuccess;
 }
 template <int NZ>
-void launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
+cudaError_t launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    static const int occ = tune("RSDFT_YZ_OCC", 4);
-    if (occ >= 6) fft3_inv_yz_kernel<NZ, 6><<<rows_grid(a, sms, 6), 128, 0, st>>>(a);
-    else if (occ == 5) fft3_inv_yz_kernel<NZ, 5><<<rows_grid(a, sms, 5), 128, 0, st>>>(a);
-    else fft3_inv_yz_kernel<NZ, 4><<<rows_grid(a, sms, 4), 128, 0, st>>>(a);
+    auto k = fft3_inv_yz_kernel<NZ>;
+    const size_t smem = ZyCfg<NZ>::SMEM_INV;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    // G x-plane walkers per row class; every walker runs over all columns of the batch
+    const int64_t gmax = std::max<int64_t>(1, (int64_t)sms * occ_by_smem(smem, 2) / a.my);
+    const int64_t rounds = (a.nx + gmax - 1) / gmax;
+    const int64_t g = (a.nx + rounds - 1) / rounds;
+    k<<<(int)(g * a.my), 128, smem, st>>>(a);
+    return cudaSuccess;
 }
 
 template <int NX, int TZ, int NT, int MINB>
 cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
 {
     const size_t smem = (size_t)NX * (a.my * TZ + 1) * sizeof(double2);
+    if (smem + 4096 > 227 * 1024) return cudaErrorInvalidConfiguration;
     const int64_t ntiles = (int64_t)a.ncol * 16 * (a.nz / TZ);
     auto k = fft3_x_kernel<NX, TZ, NT, MINB>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const int occ = (int)std::max<size_t>(1, std::min<size_t>(MINB, (227 * 1024) / (smem + 4096)));
+    const int occ = occ_by_smem(smem, MINB);
     k<<<(int)std::min<int64_t>(ntiles, (int64_t)sms * occ), NT, smem, st>>>(a);
     return cudaSuccess;
 }
@@ -425,38 +431,21 @@ cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
 template <int NX>
 cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    static const int cfg = tune("RSDFT_X_CFG", 0);
-    const size_t smem8 = (size_t)NX * (a.my * 8 + 1) * sizeof(double2);
-    if (cfg == 1) return launch_x_cfg<NX, 4, 256, 3>(a, sms, st);
-    if (cfg == 2) return launch_x_cfg<NX, 4, 128, 6>(a, sms, st);
-    if (cfg == 3) return launch_x_cfg<NX, 4, 128, 4>(a, sms, st);
-    if (2 * (smem8 + 4096) <= 227 * 1024) return launch_x_cfg<NX, 8, 256, 2>(a, sms, st);
-    return launch_x_cfg<NX, 8, 512, 1>(a, sms, st);
+    static const int var = tune("RSDFT_X_VAR", 0);      // experiments only
+    if (var == 1) return launch_x_cfg<NX, 8, 512, 1>(a, sms, st);
+    if (var == 2) return launch_x_cfg<NX, 4, 256, 2>(a, sms, st);
+    if (var == 3) return launch_x_cfg<NX, 8, 256, 2>(a, sms, st);
+    return launch_x_cfg<NX, XCfg<NX>::TZ, XCfg<NX>::NT, XCfg<NX>::MINB>(a, sms, st);
 }
 
-cudaError_t launch_x_any(int nx, const Fft3Args &a, int sms, cudaStream_t st)
-{
-    cudaError_t e = cudaErrorInvalidValue;
-    switch (nx) {
-    case 16: e = launch_x<16>(a, sms, st); break;
-    case 32: e = launch_x<32>(a, sms, st); break;
-    case 48: e = launch_x<48>(a, sms, st); break;
-    case 64: e = launch_x<64>(a, sms, st); break;
-    case 80: e = launch_x<80>(a, sms, st); break;
-    case 96: e = launch_x<96>(a, sms, st); break;
-    case 112: e = launch_x<112>(a, sms, st); break;
-    case 128: e = launch_x<128>(a, sms, st); break;
-    default: break;
-    }
-    return e;
-}
-
-template <int NP>
-void launch_project_np(const SphereTables &t, const double2 *X, int64_t ldx, int ncol, double dV, double2 *pp,
+template <int MT>
+void launch_project_mt(const SphereTables &t, const double2 *X, int64_t ldx, int ncol, double dV, double2 *pp,
                        cudaStream_t st)
 {
-    constexpr int CG = NlCols<NP>::CGP;
-    project_kernel<NP><<<dim3(t.nchunks, (ncol + CG - 1) / CG), NL_THREADS, 0, st>>>(t, X, ldx, ncol, dV, pp);
+    const int gx = (t.nchunks + 3) / 4;
+    if (ncol <= 8) project_kernel<MT, 1><<<dim3(gx, 1), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+    else if (ncol <= 16) project_kernel<MT, 2><<<dim3(gx, 1), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+    else project_kernel<MT, 4><<<dim3(gx, (ncol + 31) / 32), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
 }
 template <int NP>
 void launch_scatter_np(const SphereTables &t, int chunk0, int nlist, const double2 *q, int ncol, double2 *HX,
@@ -477,10 +466,12 @@ SphereTables sphere_tables(const rsdft_plan *P)
 
 int default_batch(const rsdft_plan *P)
 {
-    // columns per kernel sequence: keep one batch (X slice + HX slice) well inside the 126 MB L2
+    // columns per kernel sequence: ~400 MB of orbitals per launch.  Measured on B200 (configs 2-4): the
+    // kernels need >= 10-20 M points per launch to reach their asymptotic rate, and the k-space scratch
+    // stops being L2-resident beyond ~4 columns of 96^3 anyway, so small L2-sized batches only lose.
     const int64_t per_col = P->ng * 16;
-    int64_t b = (int64_t)(48ll << 20) / per_col;
-    return (int)std::max<int64_t>(1, std::min<int64_t>(b, 256));
+    int64_t b = (int64_t)(400ll << 20) / per_col;
+    return (int)std::max<int64_t>(1, std::min<int64_t>(b, 64));
 }
 
 // One batch of columns through the whole operator, on stream slot `slot`.
@@ -491,10 +482,9 @@ int apply_h_batch(rsdft_plan *P, int slot, int nb, const double2 *X, int64_t ldx
     const SphereTables tabs = sphere_tables(P);
     double2 *pp = P->pp[slot].p, *pq = P->pq[slot].p;
     if (nl) {   // projections read the INPUT orbitals
-        if (P->maxproj <= 4) launch_project_np<4>(tabs, X, ldx, nb, P->dV, pp, st);
-        else if (P->maxproj <= 9) launch_project_np<9>(tabs, X, ldx, nb, P->dV, pp, st);
-        else launch_project_np<16>(tabs, X, ldx, nb, P->dV, pp, st);
-        combine_kernel<<<dim3((nb + 127) / 128, P->natom), 128, 0, st>>>(tabs, pp, nb, pq);
+        if (P->maxproj <= 8) launch_project_mt<1>(tabs, X, ldx, nb, P->dV, pp, st);
+        else launch_project_mt<2>(tabs, X, ldx, nb, P->dV, pp, st);
+        combine_kernel<<<dim3(P->natom, (nb + NL_CCOLS - 1) / NL_CCOLS), 128, 0, st>>>(tabs, pp, nb, pq);
         P->last_launches += 2;
     }
     Fft3Args fa;
@@ -502,9 +492,13 @@ int apply_h_batch(rsdft_plan *P, int slot, int nb, const double2 *X, int64_t ldx
     fa.ncol = nb; fa.nx = Nx; fa.ny = Ny; fa.nz = Nz; fa.my = Ny / 16;
     fa.twx = P->tw[0].p; fa.twy = P->tw[1].p; fa.twz = P->tw[2].p;
     fa.kin_x = P->kin_x.p; fa.kin_yz = P->kin_yz.p; fa.vloc = P->vloc.p;
-    RS_DISPATCH_N(Nz, launch_fwd_zy, fa, P->num_sms, st)                  // z fwd, y fwd stage A:  X -> HX
-    RS_CUDA(launch_x_any(Nx, fa, P->num_sms, st));                        // y B, x fwd, t(k)/Ng, x inv, y B'
-    RS_DISPATCH_N(Nz, launch_inv_yz, fa, P->num_sms, st)                  // y A', z inv, + v(r) psi(r)
+    cudaError_t ke = cudaSuccess;
+    RS_DISPATCH_N(ke, Nz, launch_fwd_zy, fa, P->num_sms, st)              // z fwd, y fwd stage A:  X -> HX
+    RS_CUDA(ke);
+    RS_DISPATCH_N(ke, Nx, launch_x, fa, P->num_sms, st)                   // y B, x fwd, t(k)/Ng, x inv, y B'
+    RS_CUDA(ke);
+    RS_DISPATCH_N(ke, Nz, launch_inv_yz, fa, P->num_sms, st)              // y A', z inv, + v(r) psi(r)
+    RS_CUDA(ke);
     P->last_launches += 3;
     if (nl) {
         for (int c = 0; c < P->ncolour; ++c) {

@@ -143,19 +143,36 @@ def small_system(n=(12, 10, 8), L=(7.0, 6.0, 5.0), natom=3, seed=7, nproj=9, rc=
     return system
 
 
-def orbital_block(ng, cols, seed, stream, device="cpu", ld=None):
+def orbital_block(ng, cols, seed, stream, device="cpu", ld=None, out=None):
     """CN(0,1) orbitals (re, im ~ N(0, 1/2) i.i.d.; SURVEY 8(c) reading 13) as a torch
     complex128 tensor [len(cols), ld] (row c = orbital cols[c]).  Each column has its own
     generator seed (seed, stream, column), so any subset of columns can be regenerated.
     `stream` separates X (0), W (1), P (2).  Values drawn on `device`; the oracle is fed a
-    host copy of the very same tensor, never an independently drawn one."""
+    host copy of the very same tensor, never an independently drawn one.  `out` (rows of a
+    preallocated block) is filled in place instead of allocating."""
     import torch
     ld = ng if ld is None else ld
     cols = list(cols)
-    out = torch.zeros((len(cols), ld), dtype=torch.complex128, device=device)
+    if out is None:
+        out = torch.zeros((len(cols), ld), dtype=torch.complex128, device=device)
+    else:
+        device = out.device
+        assert out.shape == (len(cols), ld) and out.dtype == torch.complex128
     view = torch.view_as_real(out)
     gen = torch.Generator(device=device)
     for r, c in enumerate(cols):
         gen.manual_seed((int(seed) * 1000003 + int(stream)) * 1000003 + int(c))
         view[r, :ng, :].normal_(0.0, 0.5 ** 0.5, generator=gen)
     return out
+
+
+def block_y(system, device="cuda"):
+    """Y = [X, W, P] of a config as ONE [3m, Ng] tensor, filled block by block in place (no
+    concatenation copy: configs[4] holds 51.5 GB per block)."""
+    import torch
+    m = system["m"]
+    ng = int(np.prod(system["n"]))
+    Y = torch.empty((3 * m, ng), dtype=torch.complex128, device=device)
+    for s in range(3):
+        orbital_block(ng, range(m), system["seed"], s, out=Y[s * m:(s + 1) * m])
+    return Y

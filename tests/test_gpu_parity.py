@@ -233,3 +233,49 @@ def test_block_step_host_matches_device_path(env):
     HY = gpu_apply(env, plan, Y)
     assert torch.equal(torch.view_as_real(HY.cpu()), torch.view_as_real(HYh))
     assert rsdft.rsdft_plan_info(plan)["last_launches"] > 0
+
+
+# ------------------------------------------------------------------ BASELINE.json full sizes, bench.py's launch configuration
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_full_size_block_step_sampled_parity(env, cfg):
+    """configs[2..4] at full size (n = 3m columns, whole block resident in HBM), the library's default
+    batching/streams, i.e. exactly what bench.py times.  The oracle recomputes a seeded sample of columns
+    spread over X, W, P (HX element by element) and the matching |C| x |C| sub-blocks of H_sub and S_sub
+    over the full grid; the rest of the matrices is checked through invariants that hold at any size."""
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    system = wl.make_system(cfg)
+    m = system["m"]
+    n = 3 * m
+    ng = int(np.prod(system["n"]))
+    need = 2 * n * ng * 16 + (8 << 30)
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()                     # blocks of the previous case are still cached by torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < need:
+        pytest.skip("needs %.0f GB of free HBM" % (need / 1e9))
+    plan = rsdft.plan_from_system(system)
+    Y = wl.block_y(system, device="cuda")
+    HY = torch.empty_like(Y)
+    rsdft.rsdft_apply_h(plan, Y, HY)
+    H, S = rsdft.rsdft_subspace_gram(plan, Y, HY)
+    torch.cuda.synchronize()
+    C = sorted({0, m - 1, m, 2 * m - 3, 2 * m + 7, n - 1})
+    Yc = Y[C].cpu().numpy()
+    HY_ref = oracle.apply_h(system, Yc)
+    assert col_err(HY[C].cpu().numpy(), HY_ref) <= TOL
+    H_ref, S_ref = oracle.gram(Yc, HY_ref)
+    Hg, Sg = H.cpu().numpy().T, S.cpu().numpy().T
+    scale_h, scale_s = np.max(np.abs(Hg)), np.max(np.abs(Sg))
+    assert np.max(np.abs(Hg[np.ix_(C, C)] - H_ref)) <= TOL * scale_h
+    assert np.max(np.abs(Sg[np.ix_(C, C)] - S_ref)) <= TOL * scale_s
+    # whole-matrix properties
+    assert np.array_equal(Sg, Sg.conj().T)
+    assert np.max(np.abs(Hg - Hg.conj().T)) <= 1e-12 * scale_h
+    rows = lambda f: torch.cat([f(c0, min(c0 + 32, n)) for c0 in range(0, n, 32)]).cpu().numpy()   # chunked: no 50 GB temporaries
+    norms = rows(lambda a, b: (Y[a:b].real ** 2 + Y[a:b].imag ** 2).sum(dim=1))
+    assert np.max(np.abs(np.diagonal(Sg).real - norms)) <= 1e-12 * scale_s
+    hd = rows(lambda a, b: (Y[a:b].conj() * HY[a:b]).sum(dim=1))       # diag(H_sub) = <y_i | H y_i>
+    assert np.max(np.abs(np.diagonal(Hg) - hd)) <= 1e-12 * scale_h
+    np.linalg.cholesky(Sg)
+    plan.close()
