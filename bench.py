@@ -46,6 +46,7 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="apply_h column batch width (0 = library default)")
+    ap.add_argument("--streams", type=int, default=0, help="apply_h internal streams (0 = library default)")
     ap.add_argument("--ncol-per-call", type=int, default=0, help="columns per rsdft_apply_h call (config 4 sweep)")
     return ap.parse_args()
 
@@ -179,6 +180,16 @@ def probe_peaks():
     return out
 
 
+def ncu_traffic(cfg_id, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed
+    `ncu --set full` capture of this config (profiles/ncu_traffic.json), or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        return json.load(open(p))["config%d" % cfg_id][kernel]["dram_bytes_per_launch"]
+    except Exception:
+        return None
+
+
 def measured_peaks_file():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -226,6 +237,8 @@ def run_ours(args):
     plan = rsdft.plan_from_system(system)
     if args.batch:
         rsdft.rsdft_plan_set_batch(plan, args.batch)
+    if args.streams:
+        rsdft.rsdft_plan_set_streams(plan, args.streams)
     peaks = probe_peaks() if rank == 0 else None
 
     # Y = [X, W, P] resident in HBM (seeded per column; every rank draws the same block)
@@ -316,7 +329,8 @@ def run_ours(args):
     flops_exec = 8.0 * ng * 96 * 96 * (tm * tm + tm * (tm + 1) // 2)
     mp = measured_peaks_file()
     roofline = dict(bound="tensor", kernel="gram_dmma_kernel (FP64 DMMA.8x8x4)", achieved=flops_alg / t_gram / 1e12,
-                    peak=peaks["dmma_tflops"], unit="TFLOP/s", frac=flops_alg / t_gram / 1e12 / peaks["dmma_tflops"], traffic=None,
+                    peak=peaks["dmma_tflops"], unit="TFLOP/s", frac=flops_alg / t_gram / 1e12 / peaks["dmma_tflops"],
+                    traffic=ncu_traffic(args.config, "gram_dmma_kernel"),
                     peak_source="libpeakprobe DMMA.8x8x4 register loop on this GPU, 150 launches back to back (MEASURED_PEAKS.json "
                                 "has no FP64 entry; bf16 %.1f TF x nominal 40/2250 = %.1f TF for context)" % (
                                     (mp or {}).get("bf16_tflops", float("nan")), (mp or {}).get("bf16_tflops", float("nan")) * 40 / 2250),
@@ -324,7 +338,7 @@ def run_ours(args):
                     ms_per_launch=1e3 * t_gram)
     f_cov = rsdft.rsdft_plan_info(plan)["sphere_points"] / ng
     bytes_hx = (80.0 + 48.0 * f_cov) * ng * n                     # SURVEY 8(d) design model
-    apply_roof = dict(bound="hbm", kernels="fft_lines/fft_strided/project/scatter (rsdft_apply_h)", achieved=bytes_hx / t_apply / 1e9,
+    apply_roof = dict(bound="hbm", kernels="project/combine/fft3_fwd_zy/fft3_x/fft3_inv_yz/scatter (rsdft_apply_h)", achieved=bytes_hx / t_apply / 1e9,
                       peak=(mp or {}).get("hbm_gbs", 6650.0), peak_source="MEASURED_PEAKS.json hbm_gbs" if mp else "fallback 6650",
                       unit="GB/s", bytes_per_point=80.0 + 48.0 * f_cov, ms_per_call=1e3 * t_apply, probe_copy_gbs=peaks["copy_gbs"])
     apply_roof["frac"] = apply_roof["achieved"] / apply_roof["peak"]
@@ -337,7 +351,7 @@ def run_ours(args):
     line = dict(metric=METRIC, value=world * n * ng / (ms_per_step * 1e-3), unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64 (complex128)",
                 data="synthetic", config=dict(workload=workload_name(args.config), l2="inputs %.1f GB per block >> 126 MB L2, no flush needed" % (n * ng * 16 / 1e9),
-                                              ncol_per_apply_call=per_call, apply_batch_cols=rsdft.rsdft_plan_info(plan)["batch_cols"],
+                                              ncol_per_apply_call=per_call, apply_batch_cols=rsdft.rsdft_plan_info(plan)["batch_cols"], apply_streams=args.streams or 3,
                                               replicas=world),
                 hx_pts_per_s=n * ng / t_apply, gram_tflops=16.0 * n * n * ng / t_gram / 1e12,
                 gram_tflops_note="nominal 2*8*n^2*Ng flops / t (SURVEY 8(d)); executed flops are in roofline.executed_tflops",

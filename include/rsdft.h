@@ -128,12 +128,19 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
 
 /* Introspection used by tests/bench: fills out[0..7] with
  *   {natom, total sphere points, max points per sphere, device bytes owned by the plan,
- *    apply_h column batch width, kernels launched by the last compute call, Ng, reserved}. */
+ *    apply_h column batch width, kernels launched by the last compute call, Ng, colour classes}. */
 int rsdft_plan_info(const rsdft_plan_t *plan, int64_t *out8);
 
 /* Tuning knob: number of columns apply_h pushes through its kernel sequence at a time
- * (0 = library default, chosen so one batch stays L2-resident). */
+ * (0 = library default: about 400 MB of orbitals per launch). */
 int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols);
+
+/* Tuning knob: apply_h deals its column batches round-robin to `nstreams` plan-owned CUDA streams
+ * (forked from and joined back into the caller's stream, so the call stays asynchronous and ordered
+ * on that stream); 1 = everything on the caller's stream, 0 = library default (3), at most 4.
+ * Batches are independent, so results do not depend on this setting (bitwise).
+ * Errors: INVALID_ARG. */
+int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams);
 
 /* Destroys the plan and frees everything it owns (synchronises the device first). */
 int rsdft_plan_destroy(rsdft_plan_t *plan);

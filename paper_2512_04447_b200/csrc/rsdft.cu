@@ -97,7 +97,7 @@ struct rsdft_plan {
     static constexpr int MAX_STREAMS = 4;
     DevBuf<double2> pp[MAX_STREAMS];                  // [nchunks][maxproj][batch] partial projections
     DevBuf<double2> pq[MAX_STREAMS];                  // [natom][maxproj][batch]   q = D p
-    int nstreams = 3;                                 // batches round-robin over internal streams (RSDFT_STREAMS overrides)
+    int nstreams = 3;                                 // batches round-robin over internal streams (rsdft_plan_set_streams)
     cudaStream_t s_batch[MAX_STREAMS] = {nullptr, nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[MAX_STREAMS] = {nullptr, nullptr, nullptr, nullptr};
 
@@ -428,10 +428,28 @@ cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
     return cudaSuccess;
 }
 
+template <int NX, int NW>
+cudaError_t launch_xs(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    const size_t smem = (size_t)NX * xs_pitch(2 * a.my) * sizeof(double2);
+    auto k = fft3_xs_kernel<NX, NW>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int occ = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, NW * 32, smem);
+    if (e != cudaSuccess) return e;
+    const int64_t units = (int64_t)a.ncol * 16 * (a.nz / 2);
+    k<<<(int)std::min<int64_t>(units, (int64_t)sms * std::max(1, occ)), NW * 32, smem, st>>>(a);
+    return cudaSuccess;
+}
+
 template <int NX>
 cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 {
     static const int var = tune("RSDFT_X_VAR", 0);      // experiments only
+    if (var == 11) return launch_xs<NX, 1>(a, sms, st);
+    if (var == 12) return launch_xs<NX, 2>(a, sms, st);
+    if (var == 14) return launch_xs<NX, 4>(a, sms, st);
     if (var == 1) return launch_x_cfg<NX, 8, 512, 1>(a, sms, st);
     if (var == 2) return launch_x_cfg<NX, 4, 256, 2>(a, sms, st);
     if (var == 3) return launch_x_cfg<NX, 8, 256, 2>(a, sms, st);
@@ -442,10 +460,16 @@ template <int MT>
 void launch_project_mt(const SphereTables &t, const double2 *X, int64_t ldx, int ncol, double dV, double2 *pp,
                        cudaStream_t st)
 {
+    // widest column group (most beta/idx reuse) that still leaves >= ~8 CTAs of 4 warps per SM: the
+    // kernel is latency-bound on its gathers, so warps in flight matter more than reuse
     const int gx = (t.nchunks + 3) / 4;
-    if (ncol <= 8) project_kernel<MT, 1><<<dim3(gx, 1), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
-    else if (ncol <= 16) project_kernel<MT, 2><<<dim3(gx, 1), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
-    else project_kernel<MT, 4><<<dim3(gx, (ncol + 31) / 32), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+    const int64_t want = 148 * 8;
+    if (ncol > 16 && (int64_t)gx * ((ncol + 31) / 32) >= want)
+        project_kernel<MT, 4><<<dim3(gx, (ncol + 31) / 32), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+    else if (ncol > 8 && (int64_t)gx * ((ncol + 15) / 16) >= want)
+        project_kernel<MT, 2><<<dim3(gx, (ncol + 15) / 16), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+    else
+        project_kernel<MT, 1><<<dim3(gx, (ncol + 7) / 8), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
 }
 template <int NP>
 void launch_scatter_np(const SphereTables &t, int chunk0, int nlist, const double2 *q, int ncol, double2 *HX,
@@ -667,7 +691,6 @@ int rsdft_plan_create(const rsdft_grid_t *grid, const rsdft_box_t *box, const rs
         rc = fail(RSDFT_ALLOC, "rsdft_plan_create: host allocation failed");
     }
     if (rc != RSDFT_OK) { delete P; return rc; }
-    if (const char *e = std::getenv("RSDFT_STREAMS")) P->nstreams = std::max(1, std::min(atoi(e), (int)rsdft_plan::MAX_STREAMS));
     *out = P;
     return RSDFT_OK;
 }
@@ -693,6 +716,14 @@ int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols)
 {
     if (!plan || batch_cols < 0 || batch_cols > 65535) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_batch: bad argument");
     plan->user_batch = batch_cols;
+    return RSDFT_OK;
+}
+
+int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams)
+{
+    if (!plan || nstreams < 0 || nstreams > rsdft_plan::MAX_STREAMS)
+        return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_streams: nstreams must be in 0..4");
+    plan->nstreams = nstreams == 0 ? 3 : nstreams;
     return RSDFT_OK;
 }
 

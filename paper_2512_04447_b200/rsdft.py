@@ -5,7 +5,7 @@ if the library is missing, or it reports an error, the call raises.  torch is us
 memory and streams only (torch tensors' data_ptr() / torch.cuda.current_stream()).
 
 Function names follow the C ABI: rsdft_plan_create, rsdft_plan_set_vloc, rsdft_apply_h,
-rsdft_subspace_gram, rsdft_block_step_host, rsdft_plan_info, rsdft_plan_set_batch,
+rsdft_subspace_gram, rsdft_block_step_host, rsdft_plan_info, rsdft_plan_set_batch, rsdft_plan_set_streams,
 rsdft_plan_destroy, rsdft_last_error.  Orbital blocks are torch complex128 tensors of shape
 [ncol, ld] (row c = column c of the paper's block, contiguous in the grid index)."""
 import ctypes as C
@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librsdft.so")
 
 SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram",
-           "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_destroy",
+           "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_set_streams", "rsdft_plan_destroy",
            "rsdft_last_error"]
 
 RSDFT_OK, RSDFT_INVALID_ARG, RSDFT_UNSUPPORTED, RSDFT_ALLOC, RSDFT_CUDA = 0, -1, -2, -3, -4
@@ -74,6 +74,7 @@ def load():
     lib.rsdft_block_step_host.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32]
     lib.rsdft_plan_info.argtypes = [vp, C.POINTER(i64)]
     lib.rsdft_plan_set_batch.argtypes = [vp, i32]
+    lib.rsdft_plan_set_streams.argtypes = [vp, i32]
     lib.rsdft_plan_destroy.argtypes = [vp]
     lib.rsdft_last_error.restype = C.c_char_p
     for name in SYMBOLS:
@@ -253,6 +254,10 @@ def rsdft_plan_info(plan):
 
 def rsdft_plan_set_batch(plan, batch_cols):
     _check(load().rsdft_plan_set_batch(plan.handle, int(batch_cols)))
+
+
+def rsdft_plan_set_streams(plan, nstreams):
+    _check(load().rsdft_plan_set_streams(plan.handle, int(nstreams)))
 
 
 def rsdft_plan_destroy(plan):

@@ -130,7 +130,8 @@ def test_no_atoms_no_vloc_is_kinetic_only(env):
 @pytest.mark.parametrize("radial_kind", [0, 1])
 def test_noncubic_spd_projectors_full_D_padded_ld(env, radial_kind):
     """9 s+p+d projectors, full symmetric D, tabulated radial part, overlapping spheres, ld > Ng,
-    ncol not a multiple of the batch width; result independent of the batch width (bitwise)."""
+    ncol not a multiple of the batch width; result independent of the batch width and of the
+    number of internal streams (bitwise)."""
     torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
     system = wl.small_system(n=(32, 16, 48), L=(7.0, 4.1, 9.5), natom=5, seed=11, nproj=9, rc=1.9,
                              radial_kind=radial_kind)
@@ -140,8 +141,9 @@ def test_noncubic_spd_projectors_full_D_padded_ld(env, radial_kind):
     X = wl.orbital_block(ng, range(7), 3, 0, device="cuda", ld=ng + 24)
     ref = oracle.apply_h(system, X[:, :ng].cpu().numpy())
     outs = []
-    for batch in (0, 1, 3, 7, 16):
+    for batch, streams in ((0, 0), (1, 1), (3, 4), (7, 2), (16, 3), (2, 3)):
         rsdft.rsdft_plan_set_batch(plan, batch)
+        rsdft.rsdft_plan_set_streams(plan, streams)
         HX = gpu_apply(env, plan, X)
         assert col_err(HX[:, :ng].cpu().numpy(), ref) <= TOL
         assert bool(torch.isnan(HX[:, ng:].real).all())                 # padding untouched
