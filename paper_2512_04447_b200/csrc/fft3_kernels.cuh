@@ -126,8 +126,8 @@ __global__ void __launch_bounds__(128, MINB) fft3_fwd_zy_kernel(Fft3Args a)
 // g0, g0 + G, ...; for each plane it runs over ALL columns of the batch (the 16 rows of v(r) stay
 // hot in L1/L2).  Per tile: the k-space rows of the NEXT tile (double buffered) and the psi rows of
 // THIS tile (consumed two phases later) arrive by cp.async.
-template <int NZ>
-__global__ void __launch_bounds__(128, 2) fft3_inv_yz_kernel(Fft3Args a)
+template <int NZ, int MINB>
+__global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
 {
     constexpr int MZ = ZyCfg<NZ>::MZ, RP = ZyCfg<NZ>::RP, TILE = ZyCfg<NZ>::TILE, NT = 128;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -385,142 +385,6 @@ __global__ void __maxnreg__(((65536 / (NT * MINB)) / 8 * 8) > 255 ? 255 : ((6553
         case 6: fft3_x_store_y<6, NX, TZ, NT>(a, base, S, P, tid); break;
         case 7: fft3_x_store_y<7, NX, TZ, NT>(a, base, S, P, tid); break;
         default: fft3_x_store_y<8, NX, TZ, NT>(a, base, S, P, tid); break;
-        }
-        __syncthreads();
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// x kernel, slice form.  A CTA of NW warps owns ONE slice (column, k1y, z pair): Nx x M_y rows of
-// 32 B (one sector), i.e. lines = 2*M_y independent x-lines.  Slices never exchange data, so with
-// NW = 1 the whole pass (y stage B, x forward, t(k)/Ng, x inverse, y stage B') runs without a single
-// block barrier and the ~10 resident warps of an SM drift apart: some wait on their cp.async load
-// while others transform.  Consecutive slices are the z pairs of one (column, k1y) row group, so
-// neighbouring CTAs touch neighbouring sectors at about the same time.
-__host__ __device__ inline int xs_pitch(int lines) { return (lines % 8 == 2 || lines % 8 == 6) ? lines : lines + 2; }
-
-template <int MY, int NX, int NT>
-__device__ __forceinline__ void xs_yb_fwd(double2 *U, int P, int tid)
-{
-    for (int item = tid; item < NX * 2; item += NT) {
-        double2 *p = U + (item >> 1) * P + (item & 1);
-        double re[MY], im[MY];
-#pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = p[2 * j]; re[j] = v.x; im[j] = v.y; }
-        Dft<MY>::run(re, im);
-#pragma unroll
-        for (int j = 0; j < MY; ++j) p[2 * j] = make_double2(re[j], im[j]);
-    }
-}
-
-template <int MY, int NX, int NT>
-__device__ __forceinline__ void xs_yb_inv_store(const double2 *U, int P, int tid, double2 *base, int64_t sx, int64_t sy)
-{
-    for (int item = tid; item < NX * 2; item += NT) {
-        const int zl = item & 1, x = item >> 1;
-        const double2 *p = U + x * P + zl;
-        double re[MY], im[MY];
-#pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = p[2 * j]; re[j] = v.x; im[j] = v.y; }
-        Dft<MY>::run(im, re);
-        double2 *dst = base + x * sx + zl;
-#pragma unroll
-        for (int j = 0; j < MY; ++j) dst[j * sy] = make_double2(re[j], im[j]);
-    }
-}
-
-template <int NX, int NW>
-__global__ void __launch_bounds__(NW * 32) fft3_xs_kernel(Fft3Args a)
-{
-    constexpr int MX = NX / 16, NT = NW * 32;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2 *U = reinterpret_cast<double2 *>(smem_raw);
-    const int tid = threadIdx.x;
-    const int my = a.my, lines = 2 * my, P = xs_pitch(lines);
-    const int zpn = a.nz / 2;
-    const int64_t per_col = (int64_t)16 * zpn;
-    const int64_t units = per_col * a.ncol;
-    const int64_t sx = (int64_t)a.ny * a.nz, sy = a.nz;
-    for (int64_t u = blockIdx.x; u < units; u += gridDim.x) {
-        const int64_t colf = u / per_col;
-        const int rem = (int)(u - colf * per_col);
-        const int64_t col = a.ncol - 1 - colf;     // zig-zag: the forward kernel ended on the last column
-        const int k1y = rem / zpn, zp = rem - k1y * zpn;
-        double2 *base = a.W + col * a.ldw + (int64_t)(k1y * my) * a.nz + zp * 2;
-        for (int item = tid; item < NX * lines; item += NT) {
-            const int x = item / lines, l = item - x * lines;
-            cp_async16(U + x * P + l, base + x * sx + (l >> 1) * sy + (l & 1));
-        }
-        cp_async_commit();
-        cp_async_wait<0>();
-        __syncthreads();
-        switch (my) {
-        case 1: xs_yb_fwd<1, NX, NT>(U, P, tid); break;
-        case 2: xs_yb_fwd<2, NX, NT>(U, P, tid); break;
-        case 3: xs_yb_fwd<3, NX, NT>(U, P, tid); break;
-        case 4: xs_yb_fwd<4, NX, NT>(U, P, tid); break;
-        case 5: xs_yb_fwd<5, NX, NT>(U, P, tid); break;
-        case 6: xs_yb_fwd<6, NX, NT>(U, P, tid); break;
-        case 7: xs_yb_fwd<7, NX, NT>(U, P, tid); break;
-        default: xs_yb_fwd<8, NX, NT>(U, P, tid); break;
-        }
-        __syncthreads();
-        // x stage A: radix-MX over n1 (x = n1*16 + n2), twiddle, in place
-        for (int item = tid; item < lines * 16; item += NT) {
-            const int n2 = item / lines, l = item - n2 * lines;
-            double2 *p = U + n2 * P + l;
-            double re[MX], im[MX];
-#pragma unroll
-            for (int n1 = 0; n1 < MX; ++n1) { const double2 v = p[n1 * 16 * P]; re[n1] = v.x; im[n1] = v.y; }
-            Dft<MX>::run(re, im);
-#pragma unroll
-            for (int k = 1; k < MX; ++k) { const double2 w = __ldg(a.twx + n2 * k); tw_mul(re[k], im[k], w.x, -w.y); }
-#pragma unroll
-            for (int k = 0; k < MX; ++k) p[k * 16 * P] = make_double2(re[k], im[k]);
-        }
-        __syncthreads();
-        // x stage B (radix-16 over n2) -> frequency kx = k1 + MX*k2; kinetic factor; inverse stage B'
-        for (int item = tid; item < lines * MX; item += NT) {
-            const int k1 = item / lines, l = item - k1 * lines;
-            double2 *p = U + k1 * 16 * P + l;
-            double br[16], bi[16];
-#pragma unroll
-            for (int q = 0; q < 16; ++q) { const double2 v = p[q * P]; br[q] = v.x; bi[q] = v.y; }
-            Dft<16>::run(br, bi);
-            const double tin = __ldg(a.kin_yz + (int64_t)(k1y * my + (l >> 1)) * a.nz + zp * 2 + (l & 1));
-#pragma unroll
-            for (int k2 = 0; k2 < 16; ++k2) {
-                const double f = __ldg(a.kin_x + k1 + MX * k2) + tin;
-                br[k2] *= f; bi[k2] *= f;
-            }
-            Dft<16>::run(bi, br);                  // swapped domain from here on
-#pragma unroll
-            for (int q = 0; q < 16; ++q) p[q * P] = make_double2(br[q], bi[q]);
-        }
-        __syncthreads();
-        // x inverse stage A': conj twiddle, radix-MX over k1 -> x = n1*16 + n2
-        for (int item = tid; item < lines * 16; item += NT) {
-            const int n2 = item / lines, l = item - n2 * lines;
-            double2 *p = U + n2 * P + l;
-            double re[MX], im[MX];
-#pragma unroll
-            for (int k = 0; k < MX; ++k) { const double2 v = p[k * 16 * P]; re[k] = v.x; im[k] = v.y; }
-#pragma unroll
-            for (int k = 1; k < MX; ++k) { const double2 w = __ldg(a.twx + n2 * k); tw_mul(im[k], re[k], w.x, -w.y); }
-            Dft<MX>::run(im, re);
-#pragma unroll
-            for (int n1 = 0; n1 < MX; ++n1) p[n1 * 16 * P] = make_double2(re[n1], im[n1]);
-        }
-        __syncthreads();
-        switch (my) {
-        case 1: xs_yb_inv_store<1, NX, NT>(U, P, tid, base, sx, sy); break;
-        case 2: xs_yb_inv_store<2, NX, NT>(U, P, tid, base, sx, sy); break;
-        case 3: xs_yb_inv_store<3, NX, NT>(U, P, tid, base, sx, sy); break;
-        case 4: xs_yb_inv_store<4, NX, NT>(U, P, tid, base, sx, sy); break;
-        case 5: xs_yb_inv_store<5, NX, NT>(U, P, tid, base, sx, sy); break;
-        case 6: xs_yb_inv_store<6, NX, NT>(U, P, tid, base, sx, sy); break;
-        case 7: xs_yb_inv_store<7, NX, NT>(U, P, tid, base, sx, sy); break;
-        default: xs_yb_inv_store<8, NX, NT>(U, P, tid, base, sx, sy); break;
         }
         __syncthreads();
     }

@@ -378,12 +378,6 @@ using namespace rsdft;
     default: ERR_ = cudaErrorInvalidValue; break;                            \
     }
 
-int tune(const char *name, int dflt)
-{
-    const char *e = std::getenv(name);
-    return e ? atoi(e) : dflt;
-}
-
 // CTAs per SM that fit by shared memory (1 KB reserved per CTA), capped
 inline int occ_by_smem(size_t smem, int cap)
 {
@@ -402,7 +396,7 @@ cudaError_t launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
 template <int NZ>
 cudaError_t launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    auto k = fft3_inv_yz_kernel<NZ>;
+    auto k = fft3_inv_yz_kernel<NZ, 2>;
     const size_t smem = ZyCfg<NZ>::SMEM_INV;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -428,31 +422,9 @@ cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
     return cudaSuccess;
 }
 
-template <int NX, int NW>
-cudaError_t launch_xs(const Fft3Args &a, int sms, cudaStream_t st)
-{
-    const size_t smem = (size_t)NX * xs_pitch(2 * a.my) * sizeof(double2);
-    auto k = fft3_xs_kernel<NX, NW>;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    int occ = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, NW * 32, smem);
-    if (e != cudaSuccess) return e;
-    const int64_t units = (int64_t)a.ncol * 16 * (a.nz / 2);
-    k<<<(int)std::min<int64_t>(units, (int64_t)sms * std::max(1, occ)), NW * 32, smem, st>>>(a);
-    return cudaSuccess;
-}
-
 template <int NX>
 cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    static const int var = tune("RSDFT_X_VAR", 0);      // experiments only
-    if (var == 11) return launch_xs<NX, 1>(a, sms, st);
-    if (var == 12) return launch_xs<NX, 2>(a, sms, st);
-    if (var == 14) return launch_xs<NX, 4>(a, sms, st);
-    if (var == 1) return launch_x_cfg<NX, 8, 512, 1>(a, sms, st);
-    if (var == 2) return launch_x_cfg<NX, 4, 256, 2>(a, sms, st);
-    if (var == 3) return launch_x_cfg<NX, 8, 256, 2>(a, sms, st);
     return launch_x_cfg<NX, XCfg<NX>::TZ, XCfg<NX>::NT, XCfg<NX>::MINB>(a, sms, st);
 }
 
