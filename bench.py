@@ -313,9 +313,12 @@ def run_ours(args):
         b.record()
         barrier()
         t_e2e = max_over_ranks(max(a.elapsed_time(b) * 1e-3, 0.0)) / args.e2e_steps
-        assert torch.equal(torch.view_as_real(Hh), torch.view_as_real(Hs.cpu())), "host path and device path disagree"
+        # the host path contracts the Gram tiles panel by panel (other K split than the one-launch device path)
+        dH = float((Hh - Hs.cpu()).abs().max() / Hs.abs().max())
+        dS = float((Sh - Ss.cpu()).abs().max() / Ss.abs().max())
+        assert dH <= 1e-13 and dS <= 1e-13, "host path and device path disagree: %g %g" % (dH, dS)
         e2e = dict(value=world * n * ng / t_e2e, unit=UNIT, h2d_bytes_per_step=n * ng * 16, d2h_bytes_per_step=2 * n * n * 16,
-                   ms_per_step=1e3 * t_e2e, steps=args.e2e_steps, api="rsdft_block_step_host (pinned host Y in, H_sub/S_sub out)")
+                   ms_per_step=1e3 * t_e2e, steps=args.e2e_steps, api="rsdft_block_step_host (pinned host Y in, H_sub/S_sub out; H2D overlapped with apply_h and the panel-wise Gram)")
 
     if world > 1:
         dist.destroy_process_group()

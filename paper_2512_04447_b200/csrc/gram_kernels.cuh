@@ -33,7 +33,7 @@ struct GramArgs {
     int32_t kslabs;            // K split
     int64_t nchunks;           // Ng / KC
     const GramTile *tiles;
-    double2 *work;             // [kslabs][2][n*n] column-major partials (mat 0 = H, 1 = S)
+    double2 *work;             // [kslabs][ntiles][TN][TM] partial tiles (column-major inside a tile)
 };
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b)
@@ -144,48 +144,50 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
     cp_async_wait<0>();
 
     // epilogue: C fragment element e of (x, y) is row g, column 2t+e of that 8x8 tile
-    double2 *W = a.work + ((int64_t)ks * 2 + tl.mat) * (int64_t)a.n * a.n;
+    double2 *W = a.work + (int64_t)unit * (TM * TN);
 #pragma unroll
     for (int x = 0; x < FA; ++x)
 #pragma unroll
         for (int y = 0; y < FB; ++y)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const int i = i0 + (wm * FA + x) * 8 + g;
-                const int j = j0 + (wn * FB + y) * 8 + 2 * t + e;
-                if (i < a.n && j < a.n) W[(int64_t)j * a.n + i] = make_double2(cre[x][y][e], cim[x][y][e]);
+                const int ii = (wm * FA + x) * 8 + g;
+                const int jj = (wn * FB + y) * 8 + 2 * t + e;
+                W[jj * TM + ii] = make_double2(cre[x][y][e], cim[x][y][e]);
             }
 }
 
-// Fixed-order sum over K-slabs; H_sub written as computed, S_sub from its upper-triangular tiles:
-// element (i,j) with tile(i) < tile(j) is computed, its mirror is the conjugate; inside a diagonal
-// tile the i<j half is used and mirrored, and the diagonal's imaginary part is exactly 0
-// (S_ii = |y_i|^2), so S_sub is exactly Hermitian.
+// Fixed-order sum over K-slabs, one CTA per tile of the launch's tile list; H_sub tiles are written
+// as computed, S_sub comes from its upper-triangular tiles: element (i,j) with tile(i) < tile(j) is
+// computed, its mirror is the conjugate; inside a diagonal tile the i<j half is used and mirrored,
+// and the diagonal's imaginary part is exactly 0 (S_ii = |y_i|^2), so S_sub is exactly Hermitian.
 struct GramReduceArgs {
     const double2 *work;
+    const GramTile *tiles;
     double2 *H, *S;
-    int32_t n, lds, kslabs;
+    int32_t n, lds, kslabs, ntiles, tm, tn;
 };
 
 __global__ void __launch_bounds__(256) gram_reduce_kernel(GramReduceArgs a)
 {
-    const int64_t nn = (int64_t)a.n * a.n;
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += (int64_t)gridDim.x * blockDim.x) {
-        const int j = (int)(e / a.n), i = (int)(e - (int64_t)j * a.n);
-        if (a.H) {
-            double sr = 0.0, si = 0.0;
-            for (int k = 0; k < a.kslabs; ++k) {
-                const double2 v = a.work[((int64_t)k * 2 + 0) * nn + e];
-                sr += v.x; si += v.y;
-            }
-            a.H[(int64_t)j * a.lds + i] = make_double2(sr, si);
+    const GramTile tl = a.tiles[blockIdx.x];
+    const int i0 = tl.ti * a.tm, j0 = tl.tj * a.tn;
+    const int64_t tsz = (int64_t)a.tm * a.tn;
+    const double2 *W = a.work + (int64_t)blockIdx.x * tsz;
+    const int64_t kstride = (int64_t)a.ntiles * tsz;
+    for (int e = threadIdx.x; e < a.tm * a.tn; e += blockDim.x) {
+        const int jj = e / a.tm, ii = e - jj * a.tm;
+        const int i = i0 + ii, j = j0 + jj;
+        if (i >= a.n || j >= a.n) continue;
+        if (tl.mat == 1 && tl.ti == tl.tj && i > j) continue;
+        double sr = 0.0, si = 0.0;
+        for (int k = 0; k < a.kslabs; ++k) {
+            const double2 v = W[(int64_t)k * kstride + e];
+            sr += v.x; si += v.y;
         }
-        if (a.S && i <= j) {
-            double sr = 0.0, si = 0.0;
-            for (int k = 0; k < a.kslabs; ++k) {
-                const double2 v = a.work[((int64_t)k * 2 + 1) * nn + e];
-                sr += v.x; si += v.y;
-            }
+        if (tl.mat == 0) {
+            a.H[(int64_t)j * a.lds + i] = make_double2(sr, si);
+        } else {
             if (i == j) si = 0.0;
             a.S[(int64_t)j * a.lds + i] = make_double2(sr, si);
             if (i != j) a.S[(int64_t)i * a.lds + j] = make_double2(sr, -si);

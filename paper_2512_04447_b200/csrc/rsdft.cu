@@ -109,6 +109,9 @@ struct rsdft_plan {
     DevBuf<double2> gram_work;
     DevBuf<rsdft::GramTile> gram_tiles;
     int gram_tiles_n = -1, gram_ntiles = 0;
+    DevBuf<rsdft::GramTile> gram_panel_tiles;         // panel-ordered list of the host entry point
+    std::vector<int> gram_panel_off;
+    int gram_panel_n = -1;
 
     // host-buffer entry point
     DevBuf<double2> hostY, hostHY, hostHS;
@@ -134,7 +137,7 @@ struct rsdft_plan {
         for (int a = 0; a < 3; ++a) b += tw[a].bytes();
         b += kin_x.bytes() + kin_yz.bytes() + vloc.bytes() + pt_off.bytes() + beta_off.bytes() + idx.bytes() +
              nproj_a.bytes() + beta.bytes() + Dmat.bytes() + chunks.bytes() + atom_chunk0.bytes() + atom_chunks.bytes() +
-             gram_work.bytes() + gram_tiles.bytes() + hostY.bytes() + hostHY.bytes() + hostHS.bytes();
+             gram_work.bytes() + gram_tiles.bytes() + gram_panel_tiles.bytes() + hostY.bytes() + hostHY.bytes() + hostHS.bytes();
         for (int i = 0; i < MAX_STREAMS; ++i) b += pp[i].bytes() + pq[i].bytes();
         return b;
     }
@@ -565,6 +568,43 @@ int choose_kslabs(int64_t ntiles, int64_t nchunks, int sms)
     return best;
 }
 
+// One launch of the Gram kernels over `ntiles` tiles of a device tile list (any subset of the
+// [S|H] tiles): split-K contraction into the tile-indexed workspace, then the fixed-order reduce.
+int gram_launch(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2 *HY, int64_t ldhy, double2 *H, double2 *S,
+                int lds, const GramTile *dtiles, int ntiles, cudaStream_t st)
+{
+    if (ntiles == 0) return RSDFT_OK;
+    const int64_t nchunks = P->ng / GRAM_KC;
+    const int ks = choose_kslabs(ntiles, nchunks, P->num_sms);
+    if ((size_t)ks * ntiles * GCfg::TM * GCfg::TN > P->gram_work.n)
+        return fail(RSDFT_ALLOC, "gram_launch: workspace smaller than the launch needs (internal)");
+    GramArgs a;
+    a.Y = Y; a.HY = HY; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = ntiles; a.kslabs = ks;
+    a.nchunks = nchunks; a.tiles = dtiles; a.work = P->gram_work.p;
+    auto kern = gram_dmma_kernel<2, 4, 6, 3, 16, 3>;
+    static thread_local bool attr_set = false;
+    if (!attr_set) {
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
+        attr_set = true;
+    }
+    kern<<<ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);
+    GramReduceArgs r;
+    r.work = P->gram_work.p; r.tiles = dtiles; r.H = H; r.S = S; r.n = n; r.lds = lds; r.kslabs = ks; r.ntiles = ntiles;
+    r.tm = GCfg::TM; r.tn = GCfg::TN;
+    gram_reduce_kernel<<<ntiles, 256, 0, st>>>(r);
+    P->last_launches += 2;
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
+}
+
+// workspace elements a launch of `ntiles` tiles needs
+size_t gram_work_need(const rsdft_plan *P, int ntiles)
+{
+    if (ntiles == 0) return 0;
+    return (size_t)choose_kslabs(ntiles, P->ng / GRAM_KC, P->num_sms) * ntiles * GCfg::TM * GCfg::TN;
+}
+
+// the whole [S|H]: H tiles row-major, then the upper S tiles
 int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2 *HY, int64_t ldhy, double2 *H, double2 *S,
               int lds, cudaStream_t st)
 {
@@ -582,25 +622,26 @@ int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2
         P->gram_ntiles = (int)tiles.size();
         P->gram_tiles_n = key;
     }
-    const int64_t nchunks = P->ng / GRAM_KC;
-    const int ks = choose_kslabs(P->gram_ntiles, nchunks, P->num_sms);
-    RS_CUDA(P->gram_work.ensure((size_t)ks * 2 * n * n));
-    GramArgs a;
-    a.Y = Y; a.HY = HY; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = P->gram_ntiles; a.kslabs = ks;
-    a.nchunks = nchunks; a.tiles = P->gram_tiles.p; a.work = P->gram_work.p;
-    auto kern = gram_dmma_kernel<2, 4, 6, 3, 16, 3>;
-    static thread_local bool attr_set = false;
-    if (!attr_set) {
-        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
-        attr_set = true;
+    RS_CUDA(P->gram_work.ensure(gram_work_need(P, P->gram_ntiles)));
+    return gram_launch(P, n, Y, ldy, HY, ldhy, H, S, lds, P->gram_tiles.p, P->gram_ntiles, st);
+}
+
+// tile list ordered by column panel (panel t = tile column t): panel t holds every [S|H] tile that
+// becomes computable when columns [0, 96(t+1)) are on the device: H(i<=t, t), H(t, j<t), S(i<=t, t).
+int gram_panel_lists(rsdft_plan *P, int n)
+{
+    if (P->gram_panel_n == n) return RSDFT_OK;
+    const int tm = (n + GCfg::TM - 1) / GCfg::TM;
+    std::vector<GramTile> tiles;
+    P->gram_panel_off.assign(1, 0);
+    for (int t = 0; t < tm; ++t) {
+        for (int i = 0; i <= t; ++i) tiles.push_back({(int16_t)i, (int16_t)t, 0, 0});
+        for (int j = 0; j < t; ++j) tiles.push_back({(int16_t)t, (int16_t)j, 0, 0});
+        for (int i = 0; i <= t; ++i) tiles.push_back({(int16_t)i, (int16_t)t, 1, 0});
+        P->gram_panel_off.push_back((int)tiles.size());
     }
-    kern<<<P->gram_ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);
-    GramReduceArgs r;
-    r.work = P->gram_work.p; r.H = H; r.S = S; r.n = n; r.lds = lds; r.kslabs = ks;
-    const int64_t nn = (int64_t)n * n;
-    gram_reduce_kernel<<<(int)std::min<int64_t>((nn + 255) / 256, P->num_sms * 8), 256, 0, st>>>(r);
-    P->last_launches += 2;
-    RS_CUDA(cudaGetLastError());
+    RS_CUDA(P->gram_panel_tiles.upload(tiles));
+    P->gram_panel_n = n;
     return RSDFT_OK;
 }
 
@@ -750,15 +791,25 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     RS_CUDA(P->hostHS.ensure((size_t)2 * n * n));
     if (!P->s_copy) RS_CUDA(cudaStreamCreateWithFlags(&P->s_copy, cudaStreamNonBlocking));
     if (!P->s_comp) RS_CUDA(cudaStreamCreateWithFlags(&P->s_comp, cudaStreamNonBlocking));
-    // column chunks of ~256 MB: the H2D copy of chunk k+1 overlaps apply_h on chunk k
-    const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(n, (256ll << 20) / (ng * 16)));
+    // Column panels of one Gram tile width (96 columns): the H2D copy of panel k+1 overlaps apply_h and
+    // the Gram tiles of panel k.  After panel t has been through H, every [S|H] tile that involves only
+    // columns < 96(t+1) and touches panel t is contracted, so the Gram (the long part of the step) runs
+    // while the rest of Y is still crossing PCIe instead of after the last byte has arrived.
+    const int chunk = GCfg::TM;
     const int nchunk = (n + chunk - 1) / chunk;
     while ((int)P->ev.size() < 2 * nchunk) {
         cudaEvent_t e;
         RS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
         P->ev.push_back(e);
     }
+    int rc = gram_panel_lists(P, n);
+    if (rc != RSDFT_OK) return rc;
+    size_t need = 0;
+    for (int k = 0; k < nchunk; ++k) need = std::max(need, gram_work_need(P, P->gram_panel_off[k + 1] - P->gram_panel_off[k]));
+    RS_CUDA(P->gram_work.ensure(need));
+    double2 *Hd = P->hostHS.p, *Sd = P->hostHS.p + (size_t)n * n;
     P->last_launches = 0;
+    int64_t launches = 0;
     for (int k = 0; k < nchunk; ++k) {
         const int c0 = k * chunk, nc = std::min(chunk, n - c0);
         RS_CUDA(cudaMemcpy2DAsync(P->hostY.p + (int64_t)c0 * ng, (size_t)ng * 16,
@@ -766,15 +817,18 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
                                   cudaMemcpyHostToDevice, P->s_copy));
         RS_CUDA(cudaEventRecord(P->ev[2 * k], P->s_copy));
         RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev[2 * k], 0));
-        const int rc = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, P->s_comp);
+        rc = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, P->s_comp);
         if (rc != RSDFT_OK) return rc;
         RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], P->s_comp));
+        launches += P->last_launches;
+        P->last_launches = 0;
+        rc = gram_launch(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->gram_panel_tiles.p + P->gram_panel_off[k],
+                         P->gram_panel_off[k + 1] - P->gram_panel_off[k], P->s_comp);
+        if (rc != RSDFT_OK) return rc;
+        launches += P->last_launches;
+        P->last_launches = 0;
     }
-    const int64_t launches = P->last_launches;
-    double2 *Hd = P->hostHS.p, *Sd = P->hostHS.p + (size_t)n * n;
-    int rc = gram_impl(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->s_comp);
-    if (rc != RSDFT_OK) return rc;
-    P->last_launches += launches;
+    P->last_launches = launches;
     RS_CUDA(cudaMemcpy2DAsync(H_sub_host, (size_t)lds * 16, Hd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
     RS_CUDA(cudaMemcpy2DAsync(S_sub_host, (size_t)lds * 16, Sd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
     if (HY_host) {   // HY goes back on the copy stream, behind the uploads, while the Gram runs
