@@ -465,11 +465,11 @@ SphereTables sphere_tables(const rsdft_plan *P)
 
 int default_batch(const rsdft_plan *P)
 {
-    // columns per kernel sequence: ~400 MB of orbitals per launch.  Measured on B200 (configs 2-4): the
+    // columns per kernel sequence: ~270 MB of orbitals per launch (19 / 12 / 8 columns at 96^3 / 112^3 / 128^3).  Measured on B200 (configs 2-4): the
     // kernels need >= 10-20 M points per launch to reach their asymptotic rate, and the k-space scratch
     // stops being L2-resident beyond ~4 columns of 96^3 anyway, so small L2-sized batches only lose.
     const int64_t per_col = P->ng * 16;
-    int64_t b = (int64_t)(400ll << 20) / per_col;
+    int64_t b = (int64_t)(270ll << 20) / per_col;
     return (int)std::max<int64_t>(1, std::min<int64_t>(b, 64));
 }
 
@@ -524,28 +524,44 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
             RS_CUDA(P->pp[i].ensure((size_t)P->nchunks * P->maxproj * batch));
             RS_CUDA(P->pq[i].ensure((size_t)P->natom * P->maxproj * batch));
         }
-    if (ns > 1) {   // fork: the internal streams start after everything already queued on `st`
+    if (ns > 1) {
         if (!P->ev_fork) RS_CUDA(cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming));
         for (int i = 0; i < ns; ++i) {
             if (!P->s_batch[i]) RS_CUDA(cudaStreamCreateWithFlags(&P->s_batch[i], cudaStreamNonBlocking));
             if (!P->ev_join[i]) RS_CUDA(cudaEventCreateWithFlags(&P->ev_join[i], cudaEventDisableTiming));
         }
-        RS_CUDA(cudaEventRecord(P->ev_fork, st));
-        for (int i = 0; i < ns; ++i) RS_CUDA(cudaStreamWaitEvent(P->s_batch[i], P->ev_fork, 0));
     }
+    // With large projector tables (configs 3, 4: 43 / 98 MB of beta) the streams are re-aligned after every
+    // round of ns batches: concurrent project/scatter kernels of the ns streams then read the same beta
+    // lines through L2 (measured +6-8 %); with small tables free-running streams are as fast or faster.
+    const bool rounds = ns > 1 && P->beta.bytes() >= ((size_t)32 << 20);
+    auto fork = [&]() -> cudaError_t {      // the internal streams start after everything already queued on `st`
+        cudaError_t e = cudaEventRecord(P->ev_fork, st);
+        for (int i = 0; i < ns && e == cudaSuccess; ++i) e = cudaStreamWaitEvent(P->s_batch[i], P->ev_fork, 0);
+        return e;
+    };
+    auto join = [&]() -> cudaError_t {
+        cudaError_t e = cudaSuccess;
+        for (int i = 0; i < ns && e == cudaSuccess; ++i) {
+            e = cudaEventRecord(P->ev_join[i], P->s_batch[i]);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, P->ev_join[i], 0);
+        }
+        return e;
+    };
+    if (ns > 1) RS_CUDA(fork());
     int k = 0;
     for (int c0 = 0; c0 < ncol; c0 += batch, ++k) {
         const int nb = std::min(batch, ncol - c0);
         const int slot = ns > 1 ? k % ns : 0;
+        if (rounds && k > 0 && slot == 0) {
+            RS_CUDA(join());
+            RS_CUDA(fork());
+        }
         const int rc = apply_h_batch(P, slot, nb, X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx,
                                      ns > 1 ? P->s_batch[slot] : st);
         if (rc != RSDFT_OK) return rc;
     }
-    if (ns > 1)     // join
-        for (int i = 0; i < ns; ++i) {
-            RS_CUDA(cudaEventRecord(P->ev_join[i], P->s_batch[i]));
-            RS_CUDA(cudaStreamWaitEvent(st, P->ev_join[i], 0));
-        }
+    if (ns > 1) RS_CUDA(join());
     return RSDFT_OK;
 }
 
