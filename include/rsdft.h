@@ -110,16 +110,18 @@ int rsdft_apply_h(rsdft_plan_t *plan, int32_t ncol, const void *X, int64_t ldx,
  * (plain sums, no dV).  Y, HY: DEVICE complex128, column c at c*ldy / c*ldhy.
  * H_sub, S_sub: DEVICE, n x n complex128, column-major, element (i,j) at i + j*lds,
  * lds >= n; both triangles are written.  S_sub is exactly Hermitian; H_sub is computed in
- * full (Hermitian only to round-off).  Either of H_sub (with HY) or S_sub may be NULL to
+ * full (Hermitian only to round-off) unless rsdft_plan_set_gram_mode(plan, 1) was called.  Either of H_sub (with HY) or S_sub may be NULL to
  * skip it.  Errors: INVALID_ARG, ALLOC, CUDA. */
 int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ldy,
                         const void *HY, int64_t ldhy, void *H_sub, void *S_sub, int32_t lds,
                         void *stream);
 
-/* One whole block step with HOST buffers (the end-to-end entry point): copies Y
- * (host, pinned recommended) to the device in column chunks overlapped with rsdft_apply_h,
- * forms HY = H Y on the device, then the Gram matrices, and copies H_sub, S_sub (and HY if
- * HY_host != NULL) back to the host.  Synchronises with the host before returning.
+/* One whole block step with HOST buffers (the end-to-end entry point): copies Y (host, pinned
+ * recommended) to the device in panels of 96 columns; each panel goes through rsdft_apply_h as soon as
+ * it has arrived and then every [S|H] tile that has become computable is contracted, so both H Y and the
+ * Gram matrices overlap the rest of the upload.  Copies H_sub, S_sub (and HY if HY_host != NULL) back to
+ * the host and synchronises with the host before returning.  Results equal rsdft_apply_h +
+ * rsdft_subspace_gram on device buffers (HY bitwise; H_sub, S_sub within round-off: other K split).
  * Y_host/HY_host: HOST complex128 [n][ld]; H_sub_host, S_sub_host: HOST n x n column-major.
  * Errors: INVALID_ARG, ALLOC, CUDA. */
 int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int64_t ldy,
@@ -141,6 +143,14 @@ int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols);
  * Batches are independent, so results do not depend on this setting (bitwise).
  * Errors: INVALID_ARG. */
 int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams);
+
+/* Gram mode.  0 (default): H_sub = Y^H (HY) is contracted in full, as the definition reads (and as the
+ * paper's ZGEMM does), so it is Hermitian only to round-off.  1: only the upper 96-column
+ * tiles of H_sub are contracted and the rest is their conjugate mirror with a real diagonal, like S_sub
+ * (H is Hermitian, hence so is Y^H H Y in exact arithmetic; Hermitian eigen-solvers read one triangle
+ * anyway): 30 % fewer flops, H_sub exactly Hermitian, equal to mode 0 within round-off.
+ * Errors: INVALID_ARG. */
+int rsdft_plan_set_gram_mode(rsdft_plan_t *plan, int32_t h_upper_only);
 
 /* Destroys the plan and frees everything it owns (synchronises the device first). */
 int rsdft_plan_destroy(rsdft_plan_t *plan);

@@ -23,7 +23,7 @@
 
 namespace rsdft {
 
-struct GramTile { int16_t ti, tj, mat, pad; };   // mat 0: H_sub = Y^H HY, 1: S_sub = Y^H Y
+struct GramTile { int16_t ti, tj, mat, pad; };   // mat 0: H_sub = Y^H HY, 1: S_sub = Y^H Y (upper tile, mirrored), 2: H_sub upper tile, mirrored
 
 struct GramArgs {
     const double2 *Y, *HY;
@@ -67,8 +67,8 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
     const GramTile tl = a.tiles[unit - ks * a.ntiles];
     const int i0 = tl.ti * TM, j0 = tl.tj * TN;
     const double2 *Abase = a.Y;
-    const double2 *Bbase = tl.mat ? a.Y : a.HY;
-    const int64_t lda = a.ldy, ldb = tl.mat ? a.ldy : a.ldhy;
+    const double2 *Bbase = tl.mat == 1 ? a.Y : a.HY;
+    const int64_t lda = a.ldy, ldb = tl.mat == 1 ? a.ldy : a.ldhy;
     const int64_t c0 = a.nchunks * ks / a.kslabs, c1 = a.nchunks * (ks + 1) / a.kslabs;
     const int nch = (int)(c1 - c0);
     const int64_t r0 = c0 * KC;
@@ -161,6 +161,7 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
 // as computed, S_sub comes from its upper-triangular tiles: element (i,j) with tile(i) < tile(j) is
 // computed, its mirror is the conjugate; inside a diagonal tile the i<j half is used and mirrored,
 // and the diagonal's imaginary part is exactly 0 (S_ii = |y_i|^2), so S_sub is exactly Hermitian.
+// mat 2 applies the same rule to H_sub (optional mode: H is Hermitian, so is Y^H H Y in exact arithmetic).
 struct GramReduceArgs {
     const double2 *work;
     const GramTile *tiles;
@@ -179,7 +180,7 @@ __global__ void __launch_bounds__(256) gram_reduce_kernel(GramReduceArgs a)
         const int jj = e / a.tm, ii = e - jj * a.tm;
         const int i = i0 + ii, j = j0 + jj;
         if (i >= a.n || j >= a.n) continue;
-        if (tl.mat == 1 && tl.ti == tl.tj && i > j) continue;
+        if (tl.mat != 0 && tl.ti == tl.tj && i > j) continue;
         double sr = 0.0, si = 0.0;
         for (int k = 0; k < a.kslabs; ++k) {
             const double2 v = W[(int64_t)k * kstride + e];
@@ -188,9 +189,10 @@ __global__ void __launch_bounds__(256) gram_reduce_kernel(GramReduceArgs a)
         if (tl.mat == 0) {
             a.H[(int64_t)j * a.lds + i] = make_double2(sr, si);
         } else {
+            double2 *M = tl.mat == 1 ? a.S : a.H;          // Hermitian output: mirror the conjugate, real diagonal
             if (i == j) si = 0.0;
-            a.S[(int64_t)j * a.lds + i] = make_double2(sr, si);
-            if (i != j) a.S[(int64_t)i * a.lds + j] = make_double2(sr, -si);
+            M[(int64_t)j * a.lds + i] = make_double2(sr, si);
+            if (i != j) M[(int64_t)i * a.lds + j] = make_double2(sr, -si);
         }
     }
 }

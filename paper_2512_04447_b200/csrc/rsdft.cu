@@ -112,6 +112,7 @@ struct rsdft_plan {
     DevBuf<rsdft::GramTile> gram_panel_tiles;         // panel-ordered list of the host entry point
     std::vector<int> gram_panel_off;
     int gram_panel_n = -1;
+    int gram_h_upper = 0;                             // 1: H_sub from its upper tiles, mirrored (rsdft_plan_set_gram_mode)
 
     // host-buffer entry point
     DevBuf<double2> hostY, hostHY, hostHS;
@@ -625,12 +626,13 @@ int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2
               int lds, cudaStream_t st)
 {
     const int tm = (n + GCfg::TM - 1) / GCfg::TM;
-    const int key = n * 4 + (H ? 2 : 0) + (S ? 1 : 0);
+    const int key = n * 8 + (P->gram_h_upper ? 4 : 0) + (H ? 2 : 0) + (S ? 1 : 0);
     if (P->gram_tiles_n != key) {
         std::vector<GramTile> tiles;
         if (H)
             for (int i = 0; i < tm; ++i)
-                for (int j = 0; j < tm; ++j) tiles.push_back({(int16_t)i, (int16_t)j, 0, 0});
+                for (int j = P->gram_h_upper ? i : 0; j < tm; ++j)
+                    tiles.push_back({(int16_t)i, (int16_t)j, (int16_t)(P->gram_h_upper ? 2 : 0), 0});
         if (S)
             for (int i = 0; i < tm; ++i)
                 for (int j = i; j < tm; ++j) tiles.push_back({(int16_t)i, (int16_t)j, 1, 0});
@@ -646,18 +648,20 @@ int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2
 // becomes computable when columns [0, 96(t+1)) are on the device: H(i<=t, t), H(t, j<t), S(i<=t, t).
 int gram_panel_lists(rsdft_plan *P, int n)
 {
-    if (P->gram_panel_n == n) return RSDFT_OK;
+    const int key = 2 * n + P->gram_h_upper;
+    if (P->gram_panel_n == key) return RSDFT_OK;
     const int tm = (n + GCfg::TM - 1) / GCfg::TM;
     std::vector<GramTile> tiles;
     P->gram_panel_off.assign(1, 0);
     for (int t = 0; t < tm; ++t) {
-        for (int i = 0; i <= t; ++i) tiles.push_back({(int16_t)i, (int16_t)t, 0, 0});
-        for (int j = 0; j < t; ++j) tiles.push_back({(int16_t)t, (int16_t)j, 0, 0});
+        for (int i = 0; i <= t; ++i) tiles.push_back({(int16_t)i, (int16_t)t, (int16_t)(P->gram_h_upper ? 2 : 0), 0});
+        if (!P->gram_h_upper)
+            for (int j = 0; j < t; ++j) tiles.push_back({(int16_t)t, (int16_t)j, 0, 0});
         for (int i = 0; i <= t; ++i) tiles.push_back({(int16_t)i, (int16_t)t, 1, 0});
         P->gram_panel_off.push_back((int)tiles.size());
     }
     RS_CUDA(P->gram_panel_tiles.upload(tiles));
-    P->gram_panel_n = n;
+    P->gram_panel_n = key;
     return RSDFT_OK;
 }
 
@@ -753,6 +757,14 @@ int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams)
     if (!plan || nstreams < 0 || nstreams > rsdft_plan::MAX_STREAMS)
         return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_streams: nstreams must be in 0..4");
     plan->nstreams = nstreams == 0 ? 3 : nstreams;
+    return RSDFT_OK;
+}
+
+int rsdft_plan_set_gram_mode(rsdft_plan_t *plan, int32_t h_upper_only)
+{
+    if (!plan || (h_upper_only != 0 && h_upper_only != 1))
+        return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_gram_mode: mode must be 0 or 1");
+    plan->gram_h_upper = h_upper_only;
     return RSDFT_OK;
 }
 

@@ -6,7 +6,7 @@ memory and streams only (torch tensors' data_ptr() / torch.cuda.current_stream()
 
 Function names follow the C ABI: rsdft_plan_create, rsdft_plan_set_vloc, rsdft_apply_h,
 rsdft_subspace_gram, rsdft_block_step_host, rsdft_plan_info, rsdft_plan_set_batch, rsdft_plan_set_streams,
-rsdft_plan_destroy, rsdft_last_error.  Orbital blocks are torch complex128 tensors of shape
+rsdft_plan_set_gram_mode, rsdft_plan_destroy, rsdft_last_error.  Orbital blocks are torch complex128 tensors of shape
 [ncol, ld] (row c = column c of the paper's block, contiguous in the grid index)."""
 import ctypes as C
 import os
@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librsdft.so")
 
 SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram",
-           "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_set_streams", "rsdft_plan_destroy",
+           "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_set_streams", "rsdft_plan_set_gram_mode", "rsdft_plan_destroy",
            "rsdft_last_error"]
 
 RSDFT_OK, RSDFT_INVALID_ARG, RSDFT_UNSUPPORTED, RSDFT_ALLOC, RSDFT_CUDA = 0, -1, -2, -3, -4
@@ -75,6 +75,7 @@ def load():
     lib.rsdft_plan_info.argtypes = [vp, C.POINTER(i64)]
     lib.rsdft_plan_set_batch.argtypes = [vp, i32]
     lib.rsdft_plan_set_streams.argtypes = [vp, i32]
+    lib.rsdft_plan_set_gram_mode.argtypes = [vp, i32]
     lib.rsdft_plan_destroy.argtypes = [vp]
     lib.rsdft_last_error.restype = C.c_char_p
     for name in SYMBOLS:
@@ -258,6 +259,10 @@ def rsdft_plan_set_batch(plan, batch_cols):
 
 def rsdft_plan_set_streams(plan, nstreams):
     _check(load().rsdft_plan_set_streams(plan.handle, int(nstreams)))
+
+
+def rsdft_plan_set_gram_mode(plan, h_upper_only):
+    _check(load().rsdft_plan_set_gram_mode(plan.handle, int(h_upper_only)))
 
 
 def rsdft_plan_destroy(plan):

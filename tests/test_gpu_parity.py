@@ -281,3 +281,31 @@ def test_full_size_block_step_sampled_parity(env, cfg):
     assert np.max(np.abs(np.diagonal(Hg) - hd)) <= 1e-12 * scale_h
     np.linalg.cholesky(Sg)
     plan.close()
+
+
+def test_gram_hermitian_mode_matches_full(env):
+    """rsdft_plan_set_gram_mode(1): H_sub from its upper tiles + conjugate mirror equals the fully contracted H_sub
+    to round-off when HY really is H Y (H Hermitian), is exactly Hermitian, and matches the oracle; the host
+    entry point honours the mode too."""
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    system = wl.small_system(n=(16, 32, 16), L=(5.0, 9.0, 5.0), natom=4, seed=3, nproj=9, rc=1.6)
+    ng = 16 * 32 * 16
+    n = 200                                                   # 3 tile columns, ragged last tile
+    plan = rsdft.plan_from_system(system)
+    Y = wl.orbital_block(ng, range(n), 31, 0, device="cuda")
+    HY = gpu_apply(env, plan, Y)
+    H0, S0 = rsdft.rsdft_subspace_gram(plan, Y, HY)
+    rsdft.rsdft_plan_set_gram_mode(plan, 1)
+    H1, S1 = rsdft.rsdft_subspace_gram(plan, Y, HY)
+    torch.cuda.synchronize()
+    H0n, H1n = H0.cpu().numpy().T, H1.cpu().numpy().T
+    assert np.array_equal(H1n, H1n.conj().T) and np.all(np.diagonal(H1n).imag == 0.0)
+    assert mat_err(H1n, H0n) <= 1e-13
+    assert torch.equal(torch.view_as_real(S1), torch.view_as_real(S0))
+    Yh = Y.cpu().numpy()
+    H_ref, _ = oracle.gram(Yh, oracle.apply_h(system, Yh))
+    assert mat_err(H1n, H_ref) <= TOL
+    Hh, Sh = rsdft.rsdft_block_step_host(plan, Y.cpu().pin_memory(), None)
+    assert mat_err(Hh.numpy().T, H_ref) <= TOL
+    assert np.array_equal(Hh.numpy(), Hh.numpy().conj().T)
+    plan.close()
