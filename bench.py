@@ -200,6 +200,18 @@ def measured_peaks_file():
     return None
 
 
+def max_over_ranks_value(x, world, device):
+    """The timing rule of the multi-rank bench: every rank contributes its own device time, the job's time
+    is the maximum (all_reduce MAX over the default process group; identity at world 1)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 # ----------------------------------------------------------------------------- the CUDA arm
 def run_ours(args):
     import torch
@@ -223,11 +235,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return max_over_ranks_value(x, world, "cuda")
 
     cfg = wl.CONFIGS[args.config]
     system = wl.make_system(args.config)
