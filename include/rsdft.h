@@ -11,8 +11,9 @@
  *
  * All entry points return 0 (RSDFT_OK) or a negative rsdft_status; they never throw or
  * abort.  On error the outputs are undefined and rsdft_last_error() (thread-local) carries
- * a message.  "device" pointers are CUDA device pointers of the current device; "host"
- * pointers are ordinary host memory.  `stream` is a cudaStream_t passed as void* (NULL =
+ * a message.  "device" pointers are CUDA device pointers of the current device, which must be
+ * the device the plan was created on (INVALID_ARG otherwise); "host" pointers are ordinary
+ * host memory.  `stream` is a cudaStream_t passed as void* (NULL =
  * the legacy default stream).  The compute calls are asynchronous on `stream` and never
  * synchronise with the host; a plan owns one workspace, so at most one call per plan may
  * be in flight at a time (calls on the same stream are naturally ordered).

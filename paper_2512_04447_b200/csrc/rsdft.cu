@@ -665,6 +665,17 @@ int gram_panel_lists(rsdft_plan *P, int n)
     return RSDFT_OK;
 }
 
+// the compute calls launch on the current device: it must be the one the plan was created on
+int check_device(const rsdft_plan *P, const char *who)
+{
+    int dev = -1;
+    RS_CUDA(cudaGetDevice(&dev));
+    if (dev != P->device)
+        return fail(RSDFT_INVALID_ARG, std::string(who) + ": current CUDA device " + std::to_string(dev) +
+                                           " is not the plan's device " + std::to_string(P->device));
+    return RSDFT_OK;
+}
+
 bool overlaps(const void *a, size_t na, const void *b, size_t nb)
 {
     const char *pa = (const char *)a, *pb = (const char *)b;
@@ -785,6 +796,7 @@ int rsdft_apply_h(rsdft_plan_t *plan, int32_t ncol, const void *X, int64_t ldx, 
     if (((uintptr_t)X | (uintptr_t)HX) & 15) return fail(RSDFT_INVALID_ARG, "rsdft_apply_h: pointers must be 16-byte aligned");
     const size_t bx = ((size_t)(ncol - 1) * ldx + plan->ng) * 16, bh = ((size_t)(ncol - 1) * ldhx + plan->ng) * 16;
     if (overlaps(X, bx, HX, bh)) return fail(RSDFT_INVALID_ARG, "rsdft_apply_h: X and HX overlap");
+    if (int rc = check_device(plan, "rsdft_apply_h")) return rc;
     plan->last_launches = 0;
     return apply_h_impl(plan, ncol, (const double2 *)X, ldx, (double2 *)HX, ldhx, (cudaStream_t)stream);
 }
@@ -800,6 +812,7 @@ int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ld
     if (lds < n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: lds < n");
     if (((uintptr_t)Y | (uintptr_t)HY | (uintptr_t)H_sub | (uintptr_t)S_sub) & 15)
         return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: pointers must be 16-byte aligned");
+    if (int rc = check_device(plan, "rsdft_subspace_gram")) return rc;
     plan->last_launches = 0;
     return gram_impl(plan, n, (const double2 *)Y, ldy, H_sub ? (const double2 *)HY : nullptr, ldhy, (double2 *)H_sub,
                      (double2 *)S_sub, lds, (cudaStream_t)stream);
@@ -812,6 +825,7 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     if (n <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_block_step_host: n <= 0");
     if (ldy < plan->ng || (HY_host && ldhy < plan->ng)) return fail(RSDFT_INVALID_ARG, "rsdft_block_step_host: ld < Ng");
     if (lds < n) return fail(RSDFT_INVALID_ARG, "rsdft_block_step_host: lds < n");
+    if (int rc = check_device(plan, "rsdft_block_step_host")) return rc;
     rsdft_plan *P = plan;
     const int64_t ng = P->ng;
     RS_CUDA(P->hostY.ensure((size_t)n * ng));
