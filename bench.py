@@ -182,12 +182,16 @@ def probe_peaks():
 
 def ncu_traffic(cfg_id, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed
-    `ncu --set full` capture of this config (profiles/ncu_traffic.json), or None."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    `ncu --set full` capture of this config (profiles/ncu_traffic.csv), or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
     try:
-        return json.load(open(p))["config%d" % cfg_id][kernel]["dram_bytes_per_launch"]
+        for line in open(p).read().splitlines()[1:]:
+            f = line.split(",")
+            if int(f[0]) == cfg_id and f[1] == kernel:
+                return float(f[2])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def measured_peaks_file():
