@@ -309,3 +309,78 @@ def test_gram_hermitian_mode_matches_full(env):
     assert mat_err(Hh.numpy().T, H_ref) <= TOL
     assert np.array_equal(Hh.numpy(), Hh.numpy().conj().T)
     plan.close()
+
+
+# ------------------------------------------------------------------ properties of the CUDA operator itself (any size)
+def test_gpu_operator_is_hermitian_and_linear(env):
+    """<x|H y> = conj(<y|H x>) and H(ax + by) = a Hx + b Hy on the CUDA path (north_star's invariants, applied to
+    the product rather than the oracle): overlapping spheres, non-cubic grid with three different radix mixes."""
+    torch, rsdft, wl = env["torch"], env["rsdft"], env["wl"]
+    system = wl.small_system(n=(48, 80, 32), L=(9.0, 15.5, 6.1), natom=9, seed=21, nproj=9, rc=2.1)
+    ng = 48 * 80 * 32
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(ng, range(5), 41, 0, device="cuda")
+    Y = wl.orbital_block(ng, range(5), 41, 1, device="cuda")
+    HX, HY = gpu_apply(env, plan, X), gpu_apply(env, plan, Y)
+    A = X.conj() @ HY.T                      # A[i, j] = <x_i | H y_j>
+    B = Y.conj() @ HX.T                      # B[j, i] = <y_j | H x_i>
+    scale = float(A.abs().max())
+    assert float((A - B.conj().T).abs().max()) <= 1e-12 * scale
+    a, b = 0.7 - 1.3j, -2.1 + 0.4j
+    HZ = gpu_apply(env, plan, a * X + b * Y)
+    ref = a * HX + b * HY
+    assert float((HZ - ref).abs().max() / ref.abs().max()) <= 1e-13
+    plan.close()
+
+
+def test_gpu_translation_covariance(env):
+    """Shifting psi, v and the atoms by an integer grid vector shifts H psi identically (exercises the periodic
+    wrap of the sphere lists and of every FFT axis on the CUDA path)."""
+    torch, rsdft, wl = env["torch"], env["rsdft"], env["wl"]
+    n, L = (32, 48, 16), (8.0, 12.0, 4.0)
+    system = wl.small_system(n=n, L=L, natom=4, seed=8, nproj=4, rc=1.5)
+    ng = int(np.prod(n))
+    sh = (5, 31, 9)
+    h = [L[a] / n[a] for a in range(3)]
+    shifted = dict(system)
+    shifted["pos"] = system["pos"] + np.array([sh[a] * h[a] for a in range(3)])
+    shifted["vloc"] = np.roll(system["vloc"].reshape(n), sh, axis=(0, 1, 2)).reshape(-1).copy()
+    X = wl.orbital_block(ng, range(3), 12, 0, device="cuda")
+    Xs = torch.roll(X.reshape(3, *n), sh, dims=(1, 2, 3)).reshape(3, ng).contiguous()
+    p1, p2 = rsdft.plan_from_system(system), rsdft.plan_from_system(shifted)
+    HX = gpu_apply(env, p1, X)
+    HXs = gpu_apply(env, p2, Xs)
+    ref = torch.roll(HX.reshape(3, *n), sh, dims=(1, 2, 3)).reshape(3, ng)
+    assert float((HXs - ref).abs().max() / ref.abs().max()) <= 1e-13
+    p1.close(); p2.close()
+
+
+def test_calls_are_ordered_on_the_callers_stream(env):
+    """apply_h forks to internal streams and joins back: work queued on the caller's (non-default) stream right after
+    the call must see the finished result, and the call must wait for work queued before it."""
+    torch, rsdft, wl = env["torch"], env["rsdft"], env["wl"]
+    system = wl.make_system(1)
+    ng = 48 ** 3
+    plan = rsdft.plan_from_system(system)
+    rsdft.rsdft_plan_set_batch(plan, 4)
+    rsdft.rsdft_plan_set_streams(plan, 4)
+    X0 = wl.orbital_block(ng, range(24), 1, 0, device="cuda")
+    ref = gpu_apply(env, plan, X0)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    X = torch.zeros_like(X0)
+    HX = torch.empty_like(X0)
+    with torch.cuda.stream(side):
+        for _ in range(3):                              # keep the stream busy so ordering mistakes show
+            X.copy_(X0 * 0.0)
+            X.copy_(X0)                                 # queued BEFORE the call on the same stream
+            rsdft.rsdft_apply_h(plan, X, HX)
+            out = HX.clone()                            # queued AFTER the call on the same stream
+            H, S = rsdft.rsdft_subspace_gram(plan, X, HX)
+            Hc = H.clone()
+    side.synchronize()
+    assert torch.equal(torch.view_as_real(out), torch.view_as_real(ref))
+    H2, _ = rsdft.rsdft_subspace_gram(plan, X0, ref)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(Hc), torch.view_as_real(H2))
+    plan.close()
