@@ -117,6 +117,15 @@ int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ld
                         const void *HY, int64_t ldhy, void *H_sub, void *S_sub, int32_t lds,
                         void *stream);
 
+/* Rayleigh-Ritz update of LOBPCG (the step after the eigen-solve of the (H_sub, S_sub) pencil; Knyazev's
+ * method as cited by PAPER.md:19,124):
+ *   Out[r, j] = sum_{c < n} Y[r, c] * C[c, j],   j < m,   e.g. X' = Y C_X, HX' = HY C_X, P' = [W, P] C_P.
+ * Y: DEVICE complex128, n columns, column c at c*ldy (ldy >= Ng).  C: DEVICE complex128, n x m
+ * column-major, element (c, j) at c + j*ldc (ldc >= n).  Out: DEVICE complex128, m columns, column j at
+ * j*ldo (ldo >= Ng); must not overlap Y.  Asynchronous on `stream`.  Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+int rsdft_subspace_rotate(rsdft_plan_t *plan, int32_t n, int32_t m, const void *Y, int64_t ldy,
+                          const void *C, int32_t ldc, void *Out, int64_t ldo, void *stream);
+
 /* One whole block step with HOST buffers (the end-to-end entry point): copies Y (host, pinned
  * recommended) to the device in panels of 96 columns; each panel goes through rsdft_apply_h as soon as
  * it has arrived and then every [S|H] tile that has become computable is contracted, so both H Y and the

@@ -168,3 +168,14 @@ def gram(Y, HY=None, want_s=True):
                       _dp(S.view(np.float64)) if S is not None else None, C.c_int32(n))
     assert rc == 0
     return (H.T.copy() if H is not None else None, S.T.copy() if S is not None else None)
+
+
+def rotate(Y, Cmat):
+    """Rayleigh-Ritz update of LOBPCG (Knyazev's method, cited PAPER.md:19,124):
+    Out[j, r] = sum_c Y[c, r] * Cmat[c, j] for Y[n, Ng] (row = one column of the block) and the n x m matrix Cmat.
+    The plain definition, accumulated in long double (numpy's matmul on clongdouble is a plain loop)."""
+    Y = np.asarray(Y, dtype=np.complex128)
+    Cmat = np.asarray(Cmat, dtype=np.complex128)
+    assert Y.shape[0] == Cmat.shape[0]
+    out = Cmat.astype(np.clongdouble).T @ Y.astype(np.clongdouble)        # [m, n] @ [n, Ng]
+    return out.astype(np.complex128)

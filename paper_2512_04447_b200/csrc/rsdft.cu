@@ -18,6 +18,7 @@
 #include "fft3_kernels.cuh"
 #include "gram_kernels.cuh"
 #include "nonlocal_kernels.cuh"
+#include "rotate_kernels.cuh"
 
 namespace {
 
@@ -816,6 +817,33 @@ int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ld
     plan->last_launches = 0;
     return gram_impl(plan, n, (const double2 *)Y, ldy, H_sub ? (const double2 *)HY : nullptr, ldhy, (double2 *)H_sub,
                      (double2 *)S_sub, lds, (cudaStream_t)stream);
+}
+
+int rsdft_subspace_rotate(rsdft_plan_t *plan, int32_t n, int32_t m, const void *Y, int64_t ldy, const void *Cmat, int32_t ldc,
+                          void *Out, int64_t ldo, void *stream)
+{
+    if (!plan || !Y || !Cmat || !Out) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate: null argument");
+    if (n <= 0 || m <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate: n, m must be > 0");
+    if (ldy < plan->ng || ldo < plan->ng) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate: ld < Ng");
+    if (ldc < n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate: ldc < n");
+    if (((uintptr_t)Y | (uintptr_t)Cmat | (uintptr_t)Out) & 15)
+        return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate: pointers must be 16-byte aligned");
+    const size_t by = ((size_t)(n - 1) * ldy + plan->ng) * 16, bo = ((size_t)(m - 1) * ldo + plan->ng) * 16;
+    if (overlaps(Y, by, Out, bo)) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate: Y and Out overlap");
+    if (int rc = check_device(plan, "rsdft_subspace_rotate")) return rc;
+    using RCfg = RotateCfg<2, 4, 6, 3, 16, 3>;
+    RotateArgs a;
+    a.Y = (const double2 *)Y; a.C = (const double2 *)Cmat; a.Out = (double2 *)Out;
+    a.ldy = ldy; a.ldo = ldo; a.ng = plan->ng; a.n = n; a.m = m; a.ldc = ldc;
+    a.jtiles = (m + RCfg::TN - 1) / RCfg::TN;
+    const int64_t units = ((plan->ng + RCfg::TM - 1) / RCfg::TM) * a.jtiles;
+    if (units > 0x7fffffffll) return fail(RSDFT_UNSUPPORTED, "rsdft_subspace_rotate: too many tiles for one launch");
+    auto kern = rotate_dmma_kernel<2, 4, 6, 3, 16, 3>;
+    RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RCfg::SMEM));
+    kern<<<(unsigned)units, RCfg::THREADS, RCfg::SMEM, (cudaStream_t)stream>>>(a);
+    plan->last_launches = 1;
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
 }
 
 int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int64_t ldy, void *HY_host, int64_t ldhy,

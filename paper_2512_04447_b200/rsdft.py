@@ -5,7 +5,7 @@ if the library is missing, or it reports an error, the call raises.  torch is us
 memory and streams only (torch tensors' data_ptr() / torch.cuda.current_stream()).
 
 Function names follow the C ABI: rsdft_plan_create, rsdft_plan_set_vloc, rsdft_apply_h,
-rsdft_subspace_gram, rsdft_block_step_host, rsdft_plan_info, rsdft_plan_set_batch, rsdft_plan_set_streams,
+rsdft_subspace_gram, rsdft_subspace_rotate, rsdft_block_step_host, rsdft_plan_info, rsdft_plan_set_batch, rsdft_plan_set_streams,
 rsdft_plan_set_gram_mode, rsdft_plan_destroy, rsdft_last_error.  Orbital blocks are torch complex128 tensors of shape
 [ncol, ld] (row c = column c of the paper's block, contiguous in the grid index)."""
 import ctypes as C
@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librsdft.so")
 
-SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram",
+SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram", "rsdft_subspace_rotate",
            "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_set_streams", "rsdft_plan_set_gram_mode", "rsdft_plan_destroy",
            "rsdft_last_error"]
 
@@ -71,6 +71,7 @@ def load():
     lib.rsdft_plan_set_vloc.argtypes = [vp, vp, vp]
     lib.rsdft_apply_h.argtypes = [vp, i32, vp, i64, vp, i64, vp]
     lib.rsdft_subspace_gram.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32, vp]
+    lib.rsdft_subspace_rotate.argtypes = [vp, i32, i32, vp, i64, vp, i32, vp, i64, vp]
     lib.rsdft_block_step_host.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32]
     lib.rsdft_plan_info.argtypes = [vp, C.POINTER(i64)]
     lib.rsdft_plan_set_batch.argtypes = [vp, i32]
@@ -225,6 +226,25 @@ def rsdft_subspace_gram(plan, Y, HY, H_sub=None, S_sub=None, stream=None, want_h
                                       C.c_void_p(H_sub.data_ptr()) if want_h else None,
                                       C.c_void_p(S_sub.data_ptr()) if want_s else None, n, _stream(stream)))
     return H_sub, S_sub
+
+
+def rsdft_subspace_rotate(plan, Y, Cmat, Out=None, stream=None):
+    """Out[j, :Ng] = sum_c Cmat[c, j] * Y[c, :Ng].  Y: [n, ld] CUDA complex128 block; Cmat: torch [m, n] CUDA
+    complex128 tensor [m, ldc >= n] holding the COLUMN-MAJOR n x m matrix (Cmat_store[j, c] = C[c, j], like the
+    Gram outputs); Out: [m, ldo] block (allocated if None)."""
+    import torch
+    n, ldy = _block(Y, "Y")
+    if (not Cmat.is_cuda) or Cmat.dtype != torch.complex128 or Cmat.dim() != 2 or Cmat.stride(1) != 1 or Cmat.shape[1] < n:
+        raise ValueError("Cmat must be a CUDA complex128 tensor [m, ldc >= n] (column-major n x m)")
+    m, ldc = Cmat.shape[0], Cmat.stride(0)
+    if Out is None:
+        Out = torch.empty((m, ldy), dtype=torch.complex128, device=Y.device)
+    m2, ldo = _block(Out, "Out")
+    if m2 != m:
+        raise ValueError("Out and Cmat disagree on m")
+    _check(load().rsdft_subspace_rotate(plan.handle, n, m, C.c_void_p(Y.data_ptr()), ldy, C.c_void_p(Cmat.data_ptr()), ldc,
+                                        C.c_void_p(Out.data_ptr()), ldo, _stream(stream)))
+    return Out
 
 
 def rsdft_block_step_host(plan, Y_host, HY_host=None, H_sub_host=None, S_sub_host=None):

@@ -384,3 +384,47 @@ def test_calls_are_ordered_on_the_callers_stream(env):
     torch.cuda.synchronize()
     assert torch.equal(torch.view_as_real(Hc), torch.view_as_real(H2))
     plan.close()
+
+
+# ------------------------------------------------------------------ NEXT-2: Rayleigh-Ritz update Out = Y C
+@pytest.mark.parametrize("n,m", [(1, 1), (24, 8), (97, 50), (200, 96), (192, 200)])
+def test_rotate_parity_small_and_ragged(env, n, m):
+    """rsdft_subspace_rotate vs the oracle, element by element: ragged n (K), m (N) and a grid whose size is not a
+    multiple of the 96-point tile; padded ld on every operand."""
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    plan = rsdft.rsdft_plan_create((16, 32, 16), (5.0, 9.0, 5.0))
+    ng = 16 * 32 * 16                                       # 8192 = 85 tiles of 96 + 32
+    Y = wl.orbital_block(ng, range(n), 51, 0, device="cuda", ld=ng + 8)
+    Cs = wl.orbital_block(n, range(m), 52, 1, device="cuda", ld=n + 3)       # stored [m, ldc]: column-major n x m
+    Out = torch.full((m, ng + 16), float("nan"), dtype=torch.complex128, device="cuda")
+    rsdft.rsdft_subspace_rotate(plan, Y, Cs, Out)
+    torch.cuda.synchronize()
+    ref = oracle.rotate(Y[:, :ng].cpu().numpy(), Cs[:, :n].cpu().numpy().T)
+    assert col_err(Out[:, :ng].cpu().numpy(), ref) <= TOL
+    assert bool(torch.isnan(Out[:, ng:].real).all())        # padding untouched
+    plan.close()
+
+
+def test_rotate_full_size_config2_sampled(env):
+    """configs[2] shapes: X' = Y C_X with n = 1440, m = 480 on the 96^3 grid; the oracle recomputes a sample of
+    grid points (all 480 outputs at each) and the identity (YC)^H (YC) = C^H S_sub C ties it to the Gram kernel."""
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    system = wl.make_system(2)
+    m = system["m"]; n = 3 * m
+    ng = int(np.prod(system["n"]))
+    plan = rsdft.rsdft_plan_create(system["n"], system["len"])
+    Y = wl.block_y(system, device="cuda")
+    Cs = wl.orbital_block(n, range(m), 77, 0, device="cuda")
+    Out = rsdft.rsdft_subspace_rotate(plan, Y, Cs)
+    torch.cuda.synchronize()
+    pts = np.unique(np.concatenate([[0, 95, 96, ng - 1], np.random.default_rng(3).integers(0, ng, 60)]))
+    ref = oracle.rotate(Y[:, pts].cpu().numpy(), Cs.cpu().numpy().T)
+    got = Out[:, pts].cpu().numpy()
+    assert np.max(np.abs(got - ref)) <= TOL * np.max(np.abs(ref))
+    _, S = rsdft.rsdft_subspace_gram(plan, Y, None, want_h=False)
+    _, S2 = rsdft.rsdft_subspace_gram(plan, Out, None, want_h=False)
+    torch.cuda.synchronize()
+    Cm = Cs.cpu().numpy().T
+    want = Cm.conj().T @ S.cpu().numpy().T @ Cm
+    assert np.max(np.abs(S2.cpu().numpy().T - want)) <= 1e-11 * np.max(np.abs(want))
+    plan.close()

@@ -357,3 +357,33 @@ def test_config0_system_shapes():
     assert s["n"] == (16, 16, 16) and len(s["pos"]) == 2 and s["vloc"].shape == (4096,)
     idx, beta = oracle.sphere(s["n"], s["len"], s["pos"][0], s["species"][0])
     assert 120 <= len(idx) <= 160 and beta.shape[0] == 4     # ~137 points per sphere
+
+
+# ------------------------------------------------------------------ NEXT-2: Rayleigh-Ritz update Out = Y C
+def test_rotate_pins():
+    """oracle.rotate against what the mathematics fixes: a permutation matrix reorders columns exactly, a diagonal
+    matrix scales them, an explicit triple loop on a tiny case, linearity, and the Gram identity
+    (YC)^H (YC) = C^H (Y^H Y) C that ties it to oracle.gram (a transposed or conjugated C fails at least one)."""
+    rng = np.random.default_rng(5)
+    n, m, ng = 7, 4, 60
+    Y = rng.standard_normal((n, ng)) + 1j * rng.standard_normal((n, ng))
+    perm = [3, 0, 6, 2]
+    P = np.zeros((n, m)); P[perm, range(m)] = 1.0
+    assert np.array_equal(oracle.rotate(Y, P), Y[perm])
+    d = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    assert np.allclose(oracle.rotate(Y, np.diag(d)), d[:, None] * Y, rtol=1e-15, atol=0)
+    C = rng.standard_normal((n, m)) + 1j * rng.standard_normal((n, m))
+    out = oracle.rotate(Y, C)
+    brute = np.zeros((m, ng), dtype=complex)
+    for j in range(m):
+        for r in range(ng):
+            for c in range(n):
+                brute[j, r] += Y[c, r] * C[c, j]
+    assert np.max(np.abs(out - brute)) <= 1e-14 * np.max(np.abs(brute))
+    C2 = rng.standard_normal((n, m)) + 1j * rng.standard_normal((n, m))
+    lin = oracle.rotate(Y, 0.3 * C - 2j * C2)
+    assert np.max(np.abs(lin - (0.3 * out - 2j * oracle.rotate(Y, C2)))) <= 1e-14 * np.max(np.abs(lin))
+    _, S = oracle.gram(Y, None)
+    _, S_rot = oracle.gram(out, None)
+    ref = C.conj().T @ S @ C
+    assert np.max(np.abs(S_rot - ref)) <= 1e-13 * np.max(np.abs(ref))
