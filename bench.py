@@ -320,6 +320,25 @@ def run_ours(args):
     assert dHu <= 1e-13, "Hermitian-mode H_sub differs from the full contraction: %g" % dHu
     del Hs2
 
+    # ---- NEXT-2: the Rayleigh-Ritz update X' = Y C_X on the same block; informational
+    rot = None
+    free_b, _ = torch.cuda.mem_get_info()
+    if free_b > (m * ng * 16 + (4 << 30)):
+        Cx = wl.orbital_block(n, range(m), system["seed"], 7, device="cuda")       # [m, n]: column-major n x m
+        Xn = torch.empty((m, ng), dtype=torch.complex128, device="cuda")
+        rsdft.rsdft_subspace_rotate(plan, Y, Cx, Xn)
+        r0 = torch.cuda.Event(enable_timing=True); r1 = torch.cuda.Event(enable_timing=True)
+        r0.record()
+        for _ in range(3):
+            rsdft.rsdft_subspace_rotate(plan, Y, Cx, Xn)
+        r1.record()
+        torch.cuda.synchronize()
+        t_rot = r0.elapsed_time(r1) / 3 * 1e-3
+        rot = dict(ms=1e3 * t_rot, tflops=8.0 * ng * n * m / t_rot / 1e12,
+                   frac_of_dmma_peak=(8.0 * ng * n * m / t_rot / 1e12 / peaks["dmma_tflops"]) if peaks else None, shape="Out[Ng x %d] = Y[Ng x %d] C[%d x %d]" % (m, n, n, m),
+                   note="rsdft_subspace_rotate, one call (X' = Y C_X); flops 8*Ng*n*m")
+        del Cx, Xn
+
     # ---- end to end through the host-buffer entry point (N replicas, same max-over-ranks rule)
     e2e = None
     if not args.no_e2e:
@@ -391,6 +410,7 @@ def run_ours(args):
                                          value=world * n * ng / (t_apply + t_gram_hu), max_rel_diff_vs_full=dHu,
                                          note="rsdft_plan_set_gram_mode(1): H_sub upper tiles + conjugate mirror (30 % fewer flops); "
                                               "informational, the headline uses the full contraction"),
+                next2_rotate=rot,
                 clocks=clocks, e2e=e2e, gpu_launches=gpu_launches, cpu_baseline=cpu,
                 peaks_probe=peaks)
     print(json.dumps(line))
