@@ -831,16 +831,26 @@ int rsdft_subspace_rotate(rsdft_plan_t *plan, int32_t n, int32_t m, const void *
     const size_t by = ((size_t)(n - 1) * ldy + plan->ng) * 16, bo = ((size_t)(m - 1) * ldo + plan->ng) * 16;
     if (overlaps(Y, by, Out, bo)) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate: Y and Out overlap");
     if (int rc = check_device(plan, "rsdft_subspace_rotate")) return rc;
-    using RCfg = RotateCfg<2, 4, 6, 3, 16, 3>;
     RotateArgs a;
     a.Y = (const double2 *)Y; a.C = (const double2 *)Cmat; a.Out = (double2 *)Out;
     a.ldy = ldy; a.ldo = ldo; a.ng = plan->ng; a.n = n; a.m = m; a.ldc = ldc;
-    a.jtiles = (m + RCfg::TN - 1) / RCfg::TN;
-    const int64_t units = ((plan->ng + RCfg::TM - 1) / RCfg::TM) * a.jtiles;
+    // output tile 96 x 96 or 64 x 128 (rows x columns), whichever pads m less (m = 480 -> 96, m = 512 -> 128)
+    const bool wide = ((m + 127) / 128) * 128 < ((m + 95) / 96) * 96;
+    using R96 = RotateCfg<2, 4, 6, 3, 16, 3>;
+    using R128 = RotateCfg<2, 4, 4, 4, 16, 3>;
+    const int tm = wide ? R128::TM : R96::TM, tn = wide ? R128::TN : R96::TN;
+    a.jtiles = (m + tn - 1) / tn;
+    const int64_t units = ((plan->ng + tm - 1) / tm) * a.jtiles;
     if (units > 0x7fffffffll) return fail(RSDFT_UNSUPPORTED, "rsdft_subspace_rotate: too many tiles for one launch");
-    auto kern = rotate_dmma_kernel<2, 4, 6, 3, 16, 3>;
-    RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RCfg::SMEM));
-    kern<<<(unsigned)units, RCfg::THREADS, RCfg::SMEM, (cudaStream_t)stream>>>(a);
+    if (wide) {
+        auto kern = rotate_dmma_kernel<2, 4, 4, 4, 16, 3>;
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R128::SMEM));
+        kern<<<(unsigned)units, R128::THREADS, R128::SMEM, (cudaStream_t)stream>>>(a);
+    } else {
+        auto kern = rotate_dmma_kernel<2, 4, 6, 3, 16, 3>;
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R96::SMEM));
+        kern<<<(unsigned)units, R96::THREADS, R96::SMEM, (cudaStream_t)stream>>>(a);
+    }
     plan->last_launches = 1;
     RS_CUDA(cudaGetLastError());
     return RSDFT_OK;

@@ -387,7 +387,7 @@ def test_calls_are_ordered_on_the_callers_stream(env):
 
 
 # ------------------------------------------------------------------ NEXT-2: Rayleigh-Ritz update Out = Y C
-@pytest.mark.parametrize("n,m", [(1, 1), (24, 8), (97, 50), (200, 96), (192, 200)])
+@pytest.mark.parametrize("n,m", [(1, 1), (24, 8), (97, 50), (200, 96), (192, 200), (40, 128), (33, 250)])
 def test_rotate_parity_small_and_ragged(env, n, m):
     """rsdft_subspace_rotate vs the oracle, element by element: ragged n (K), m (N) and a grid whose size is not a
     multiple of the 96-point tile; padded ld on every operand."""
