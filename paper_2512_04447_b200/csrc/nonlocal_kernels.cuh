@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(128) combine_kernel(SphereTables t, const doub
         const int i = e / nc, c = e - i * nc;
         double sr = 0.0, si = 0.0;
         for (int j = 0; j < np; ++j) {
-            const double d = D[i * np + j];
+            const double d = D[i * mp + j];          // rows of D are stored with stride maxproj
             sr = fma(d, ps[j][c].x, sr);
             si = fma(d, ps[j][c].y, si);
         }

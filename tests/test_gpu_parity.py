@@ -428,3 +428,20 @@ def test_rotate_full_size_config2_sampled(env):
     want = Cm.conj().T @ S.cpu().numpy().T @ Cm
     assert np.max(np.abs(S2.cpu().numpy().T - want)) <= 1e-11 * np.max(np.abs(want))
     plan.close()
+
+
+def test_two_species_with_different_projector_counts(env):
+    """Atoms of two species (4 s+p projectors with a diagonal D, 9 s+p+d projectors with a full symmetric D,
+    different cut-off radii) in one plan: the per-atom projector count is smaller than the plan's maximum."""
+    oracle, rsdft, wl = env["oracle"], env["rsdft"], env["wl"]
+    a = wl.small_system(n=(32, 32, 16), L=(7.0, 7.5, 4.0), natom=6, seed=17, nproj=9, rc=1.7)
+    b = wl.small_system(n=(32, 32, 16), L=(7.0, 7.5, 4.0), natom=6, seed=18, nproj=4, rc=1.3)
+    system = dict(a)
+    system["species"] = [a["species"][0], b["species"][0]]
+    system["species_of"] = np.array([0, 1, 1, 0, 1, 0], np.int32)
+    ng = 32 * 32 * 16
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(ng, range(9), 4, 0, device="cuda")
+    HX = gpu_apply(env, plan, X)
+    assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
+    plan.close()
