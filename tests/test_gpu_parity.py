@@ -445,3 +445,41 @@ def test_two_species_with_different_projector_counts(env):
     HX = gpu_apply(env, plan, X)
     assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
     plan.close()
+
+
+def test_rayleigh_ritz_chain_recovers_free_electron_levels(env):
+    """apply_h -> gram -> (host eigh of the small pencil) -> rotate, chained on the GPU path: for V = 0 and no
+    projectors a subspace spanned by plane waves is invariant, so one Rayleigh-Ritz step must return the
+    free-electron levels 1/2 |G|^2 (closed form; north_star's Ritz-value pin) with vanishing residuals
+    H x' - lambda x', whatever (well-conditioned) mixture of the plane waves the block Y holds."""
+    import scipy.linalg
+    torch, rsdft = env["torch"], env["rsdft"]
+    n3, L = (16, 16, 32), (10.0, 10.0, 12.0)
+    ng = int(np.prod(n3))
+    rng = np.random.default_rng(11)
+    ks = set()
+    while len(ks) < 24:
+        ks.add(tuple(int(v) for v in rng.integers(0, [16, 16, 32])))
+    ks = sorted(ks)
+    ii = np.indices(n3).reshape(3, -1)
+    PW = np.stack([np.exp(2j * np.pi * sum(k[a] * ii[a] / n3[a] for a in range(3))) for k in ks]) / np.sqrt(ng)
+    M = rng.standard_normal((24, 24)) + 1j * rng.standard_normal((24, 24)) + 4.0 * np.eye(24)
+    plan = rsdft.rsdft_plan_create(n3, L)
+    Y = torch.as_tensor(M @ PW).cuda()
+    HY = gpu_apply(env, plan, Y)
+    H, S = rsdft.rsdft_subspace_gram(plan, Y, HY)
+    torch.cuda.synchronize()
+    w, V = scipy.linalg.eigh(H.cpu().numpy().T, S.cpu().numpy().T)       # the NEXT-1 step, on the host here
+    kap = lambda j, N: j if 2 * j < N else j - N
+    t = np.sort([0.5 * sum((2 * np.pi * kap(k[a], n3[a]) / L[a]) ** 2 for a in range(3)) for k in ks])
+    assert np.max(np.abs(w - t)) <= 1e-11 * t.max()
+    m = 8
+    Cs = torch.as_tensor(np.ascontiguousarray(V[:, :m].T)).cuda()            # [m, n]: column-major n x m
+    Xn = rsdft.rsdft_subspace_rotate(plan, Y, Cs)
+    HXn = rsdft.rsdft_subspace_rotate(plan, HY, Cs)
+    torch.cuda.synchronize()
+    R = HXn.cpu().numpy() - w[:m, None] * Xn.cpu().numpy()
+    assert np.max(np.abs(R)) <= 1e-10 * t.max() * np.max(np.abs(Xn.cpu().numpy()))
+    HXn2 = gpu_apply(env, plan, Xn)                                           # H (Y C) == (H Y) C
+    assert float((HXn2 - HXn).abs().max() / HXn.abs().max()) <= 1e-12
+    plan.close()
