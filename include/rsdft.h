@@ -30,7 +30,7 @@ extern "C" {
 typedef enum {
     RSDFT_OK = 0,
     RSDFT_INVALID_ARG = -1, /* null pointer, ncol <= 0, ld < Ng, X aliases HX, |m| > l, l > 2, ... */
-    RSDFT_UNSUPPORTED = -2, /* grid length outside {16,32,48,64,80,96,112,128}; box <= 0; 2*rc >= min L */
+    RSDFT_UNSUPPORTED = -2, /* grid length outside {16,...,128 step 16, 160, 192, 256}; box <= 0; 2*rc >= min L */
     RSDFT_ALLOC = -3,       /* host or device allocation failed */
     RSDFT_CUDA = -4         /* CUDA runtime error; message carries cudaGetErrorString */
 } rsdft_status;

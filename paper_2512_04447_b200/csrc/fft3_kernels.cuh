@@ -3,7 +3,7 @@
 // SURVEY 8(a) a1-a4).  One HBM/L2 round trip per kernel: 3 x (16 + 16) B per orbital*point, plus
 // the 16 B re-read of psi for v(r) psi(r).
 //
-// Every axis length is N = 16*M (M = 1..8).  Two 1-D decompositions are used (W_N = e^{-2 pi i/N}):
+// Every axis length is N = 16*M (M = 1..8, 10, 12, 16).  Two 1-D decompositions are used (W_N = e^{-2 pi i/N}):
 //   "M-first"  (z and x axes):  n = n1*16 + n2,  k = k1 + M*k2,
 //        X[k] = sum_n2 W_16^{n2 k2} [ W_N^{n2 k1} sum_n1 W_M^{n1 k1} x[n1*16 + n2] ]
 //        stage A = radix-M over n1 (+ twiddle), stage B = radix-16 over n2; in place, so k-space
@@ -52,6 +52,7 @@ struct ZyCfg {
     static constexpr int MZ = NZ / 16;
     static constexpr int RP = MZ * 17;                 // smem row pitch: 17 slots per 16-point group
     static constexpr int TILE = 16 * RP;               // double2 elements per tile buffer
+    static constexpr size_t SMEM_FWD = (size_t)TILE * sizeof(double2);
     static constexpr size_t SMEM_INV = (size_t)(2 * TILE + 16 * NZ) * sizeof(double2);
 };
 
@@ -62,7 +63,8 @@ __global__ void __launch_bounds__(128, MINB) fft3_fwd_zy_kernel(Fft3Args a)
     constexpr int MZ = NZ / 16;
     constexpr int RP = MZ * 17;                 // smem row pitch: 17 slots per 16-point group
     constexpr int NT = 128;
-    __shared__ double2 S[16 * RP];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2 *S = reinterpret_cast<double2 *>(smem_raw);          // [16 * RP]
     __shared__ double2 twz_s[(MZ > 1 ? MZ - 1 : 1) * 16];
     __shared__ double2 twy_s[16];
     const int tid = threadIdx.x;
@@ -294,6 +296,9 @@ template <> struct XCfg<80> { static constexpr int TZ = 8, NT = 224, MINB = 2; }
 template <> struct XCfg<96> { static constexpr int TZ = 8, NT = 256, MINB = 2; };
 template <> struct XCfg<112> { static constexpr int TZ = 8, NT = 256, MINB = 2; };
 template <> struct XCfg<128> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
+template <> struct XCfg<160> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
+template <> struct XCfg<192> { static constexpr int TZ = 4, NT = 256, MINB = 1; };
+template <> struct XCfg<256> { static constexpr int TZ = 2, NT = 256, MINB = 1; };
 
 template <int NX, int TZ, int NT, int MINB>
 __global__ void __maxnreg__(((65536 / (NT * MINB)) / 8 * 8) > 255 ? 255 : ((65536 / (NT * MINB)) / 8 * 8)) fft3_x_kernel(Fft3Args a)
@@ -325,7 +330,10 @@ __global__ void __maxnreg__(((65536 / (NT * MINB)) / 8 * 8) > 255 ? 255 : ((6553
         case 5: fft3_x_load_y<5, NX, TZ, NT>(a, base, S, P, tid); break;
         case 6: fft3_x_load_y<6, NX, TZ, NT>(a, base, S, P, tid); break;
         case 7: fft3_x_load_y<7, NX, TZ, NT>(a, base, S, P, tid); break;
-        default: fft3_x_load_y<8, NX, TZ, NT>(a, base, S, P, tid); break;
+        case 8: fft3_x_load_y<8, NX, TZ, NT>(a, base, S, P, tid); break;
+        case 10: fft3_x_load_y<10, NX, TZ, NT>(a, base, S, P, tid); break;
+        case 12: fft3_x_load_y<12, NX, TZ, NT>(a, base, S, P, tid); break;
+        default: fft3_x_load_y<16, NX, TZ, NT>(a, base, S, P, tid); break;
         }
         __syncthreads();
         // x stage A: radix-MX over n1 (x = n1*16 + n2), twiddle, in place
@@ -384,7 +392,10 @@ __global__ void __maxnreg__(((65536 / (NT * MINB)) / 8 * 8) > 255 ? 255 : ((6553
         case 5: fft3_x_store_y<5, NX, TZ, NT>(a, base, S, P, tid); break;
         case 6: fft3_x_store_y<6, NX, TZ, NT>(a, base, S, P, tid); break;
         case 7: fft3_x_store_y<7, NX, TZ, NT>(a, base, S, P, tid); break;
-        default: fft3_x_store_y<8, NX, TZ, NT>(a, base, S, P, tid); break;
+        case 8: fft3_x_store_y<8, NX, TZ, NT>(a, base, S, P, tid); break;
+        case 10: fft3_x_store_y<10, NX, TZ, NT>(a, base, S, P, tid); break;
+        case 12: fft3_x_store_y<12, NX, TZ, NT>(a, base, S, P, tid); break;
+        default: fft3_x_store_y<16, NX, TZ, NT>(a, base, S, P, tid); break;
         }
         __syncthreads();
     }

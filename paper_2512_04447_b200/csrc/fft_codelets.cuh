@@ -50,6 +50,14 @@ template <> struct Trig<8> {
     static constexpr double s[8] = {0.0, 0.707106781186547524401, 1.0, 0.707106781186547524401,
                                     0.0, -0.707106781186547524401, -1.0, -0.707106781186547524401};
 };
+template <> struct Trig<10> {
+    static constexpr double c[10] = {1.00000000000000000000, 0.809016994374947424102, 0.309016994374947424102, -0.309016994374947424102, -0.809016994374947424102, -1.00000000000000000000, -0.809016994374947424102, -0.309016994374947424102, 0.309016994374947424102, 0.809016994374947424102};
+    static constexpr double s[10] = {0.0, 0.587785252292473129169, 0.951056516295153572116, 0.951056516295153572116, 0.587785252292473129169, 0.0, -0.587785252292473129169, -0.951056516295153572116, -0.951056516295153572116, -0.587785252292473129169};
+};
+template <> struct Trig<12> {
+    static constexpr double c[12] = {1.00000000000000000000, 0.866025403784438646764, 0.500000000000000000000, 0.0, -0.500000000000000000000, -0.866025403784438646764, -1.00000000000000000000, -0.866025403784438646764, -0.500000000000000000000, 0.0, 0.500000000000000000000, 0.866025403784438646764};
+    static constexpr double s[12] = {0.0, 0.500000000000000000000, 0.866025403784438646764, 1.00000000000000000000, 0.866025403784438646764, 0.500000000000000000000, 0.0, -0.500000000000000000000, -0.866025403784438646764, -1.00000000000000000000, -0.866025403784438646764, -0.500000000000000000000};
+};
 template <> struct Trig<16> {
     static constexpr double c[16] = {1.0, 0.923879532511286756128, 0.707106781186547524401, 0.382683432365089771728,
                                      0.0, -0.382683432365089771728, -0.707106781186547524401, -0.923879532511286756128,
@@ -198,6 +206,8 @@ struct DftCT {
 };
 template <> struct Dft<6> : DftCT<2, 3> {};
 template <> struct Dft<8> : DftCT<2, 4> {};
+template <> struct Dft<10> : DftCT<2, 5> {};
+template <> struct Dft<12> : DftCT<3, 4> {};
 template <> struct Dft<16> : DftCT<4, 4> {};
 
 }  // namespace rsdft

@@ -380,6 +380,9 @@ using namespace rsdft;
     case 96: ERR_ = FN_<96>(__VA_ARGS__); break;                             \
     case 112: ERR_ = FN_<112>(__VA_ARGS__); break;                           \
     case 128: ERR_ = FN_<128>(__VA_ARGS__); break;                           \
+    case 160: ERR_ = FN_<160>(__VA_ARGS__); break;                           \
+    case 192: ERR_ = FN_<192>(__VA_ARGS__); break;                           \
+    case 256: ERR_ = FN_<256>(__VA_ARGS__); break;                           \
     default: ERR_ = cudaErrorInvalidValue; break;                            \
     }
 
@@ -392,10 +395,14 @@ inline int occ_by_smem(size_t smem, int cap)
 template <int NZ>
 cudaError_t launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    // G plane-walkers for each of the my row classes, two CTA generations of 4 per SM
+    auto k = fft3_fwd_zy_kernel<NZ, 4>;
+    const size_t smem = ZyCfg<NZ>::SMEM_FWD;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    // G plane-walkers for each of the my row classes, two CTA generations of the resident set
     const int64_t planes = (int64_t)a.ncol * a.nx;
-    const int64_t g = std::max<int64_t>(1, std::min<int64_t>(planes, (int64_t)sms * 8 / a.my));
-    fft3_fwd_zy_kernel<NZ, 4><<<(int)(g * a.my), 128, 0, st>>>(a);
+    const int64_t g = std::max<int64_t>(1, std::min<int64_t>(planes, (int64_t)sms * 2 * occ_by_smem(smem, 4) / a.my));
+    k<<<(int)(g * a.my), 128, smem, st>>>(a);
     return cudaSuccess;
 }
 template <int NZ>
@@ -430,7 +437,11 @@ cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
 template <int NX>
 cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    return launch_x_cfg<NX, XCfg<NX>::TZ, XCfg<NX>::NT, XCfg<NX>::MINB>(a, sms, st);
+    // the tile is NX x (my*TZ) elements: fall back to narrower z chunks when a large ny makes it too big
+    auto fits = [&](int tz) { return (size_t)NX * (a.my * tz + 1) * sizeof(double2) + 4096 <= (size_t)227 * 1024; };
+    if (fits(XCfg<NX>::TZ)) return launch_x_cfg<NX, XCfg<NX>::TZ, XCfg<NX>::NT, XCfg<NX>::MINB>(a, sms, st);
+    if (fits(4)) return launch_x_cfg<NX, 4, 256, 1>(a, sms, st);
+    return launch_x_cfg<NX, 2, 256, 1>(a, sms, st);
 }
 
 template <int MT>
@@ -700,9 +711,10 @@ int rsdft_plan_create(const rsdft_grid_t *grid, const rsdft_box_t *box, const rs
     for (int a = 0; a < 3; ++a) {
         const int N = grid->n[a];
         if (N <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: grid length <= 0");
-        if (N % 16 != 0 || N > 128)
+        const int M = N / 16;
+        if (N % 16 != 0 || !(M <= 8 || M == 10 || M == 12 || M == 16))
             return fail(RSDFT_UNSUPPORTED, "rsdft_plan_create: grid length " + std::to_string(N) +
-                                               " not in {16,32,48,64,80,96,112,128}");
+                                               " not in {16,32,48,64,80,96,112,128,160,192,256}");
         if (!(box->len[a] > 0.0) || !std::isfinite(box->len[a]))
             return fail(RSDFT_UNSUPPORTED, "rsdft_plan_create: box length must be positive and finite");
     }

@@ -5,8 +5,8 @@ FFT, i.e. two 3-D transforms per orbital).
 
     python -m paper_2512_04447_b200.fft_sweep [--grids 32,48,...] [--batches 1,512] [--reps 20]
 
-Prints one JSON line per (grid, batch).  Grids outside 16*M, M <= 8 are not supported by the library yet
-(the paper's sweep reaches 256^3)."""
+Prints one JSON line per (grid, batch).  Supported lengths: 16*M, M in {1..8, 10, 12, 16} (the paper's sweep
+reaches 256^3: use e.g. --grids 160,192,256 --batches 1,64 there, 512 orbitals of 256^3 do not fit)."""
 import argparse
 import json
 

@@ -88,7 +88,7 @@ def test_apply_h_only_x_block_config0(env):
 
 
 # ------------------------------------------------------------------ every supported length on every axis
-@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 112, 128])
+@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 112, 128, 160, 192, 256])
 @pytest.mark.parametrize("axis", [0, 1, 2])
 def test_kinetic_every_length_every_axis(env, N, axis):
     torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
@@ -482,4 +482,19 @@ def test_rayleigh_ritz_chain_recovers_free_electron_levels(env):
     assert np.max(np.abs(R)) <= 1e-10 * t.max() * np.max(np.abs(Xn.cpu().numpy()))
     HXn2 = gpu_apply(env, plan, Xn)                                           # H (Y C) == (H Y) C
     assert float((HXn2 - HXn).abs().max() / HXn.abs().max()) <= 1e-12
+    plan.close()
+
+
+@pytest.mark.parametrize("n3", [(112, 256, 16), (256, 16, 192), (16, 160, 256)])
+def test_mixed_large_lengths_with_projectors(env, n3):
+    """Lengths 160, 192, 256 (M = 10, 12, 16) mixed with small ones, projectors included: exercises the x kernel's
+    narrower-tile fallback for a large ny and the one-CTA-per-SM shapes of the 256-point kernels."""
+    oracle, rsdft, wl = env["oracle"], env["rsdft"], env["wl"]
+    L = tuple(0.21 * v for v in n3)
+    system = wl.small_system(n=n3, L=L, natom=3, seed=9, nproj=4, rc=1.2)
+    ng = int(np.prod(n3))
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(ng, range(2), 14, 0, device="cuda")
+    HX = gpu_apply(env, plan, X)
+    assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
     plan.close()
