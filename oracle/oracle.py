@@ -20,16 +20,17 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rsdft_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "rsdft_eig_oracle.c")]
 _LIB = os.path.join(_HERE, "librsdft_oracle.so")
 _lib = None
 
 
 def build(force=False):
-    """Compile rsdft_oracle.c with gcc (-O2, OpenMP, no fast-math)."""
-    if (not force) and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
+    """Compile rsdft_oracle.c and rsdft_eig_oracle.c with gcc (-O2, OpenMP, no fast-math)."""
+    if (not force) and os.path.exists(_LIB) and all(os.path.getmtime(_LIB) >= os.path.getmtime(s) for s in _SRCS):
         return _LIB
-    cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall",
-           "-o", _LIB, _SRC, "-lm"]
+    cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=gnu11", "-Wall",
+           "-o", _LIB] + _SRCS + ["-lm"]
     subprocess.check_call(cmd)
     return _LIB
 
@@ -179,3 +180,109 @@ def rotate(Y, Cmat):
     assert Y.shape[0] == Cmat.shape[0]
     out = Cmat.astype(np.clongdouble).T @ Y.astype(np.clongdouble)        # [m, n] @ [n, Ng]
     return out.astype(np.complex128)
+
+
+# ----------------------------------------------------------------------------- NEXT-1 / NEXT-2
+def _cm(a):
+    """numpy M[i, j] -> column-major buffer (element (i, j) at i + j*n) as a contiguous array"""
+    return np.ascontiguousarray(np.asarray(a, dtype=np.complex128).T)
+
+
+def potrf(S):
+    """Cholesky factor L (lower, real positive diagonal) of the Hermitian positive definite S = L L^H
+    (PAPER.md:22); plain column algorithm in long double.  Raises if S is not positive definite."""
+    S = np.asarray(S, dtype=np.complex128)
+    n = S.shape[0]
+    Sb = _cm(S)
+    Lb = np.zeros((n, n), dtype=np.complex128)
+    rc = _load().orc_potrf(C.c_int32(n), _dp(Sb.view(np.float64)), C.c_int32(n), _dp(Lb.view(np.float64)), C.c_int32(n))
+    if rc != 0:
+        raise np.linalg.LinAlgError("oracle.potrf: pivot %d is not positive" % rc)
+    return Lb.T.copy()
+
+
+def reduce_to_standard(H, S):
+    """K = L^-1 H L^-H with S = L L^H, by two triangular substitutions (eq. 1)."""
+    H = np.asarray(H, dtype=np.complex128)
+    n = H.shape[0]
+    Hb, Sb = _cm(H), _cm(S)
+    Kb = np.zeros((n, n), dtype=np.complex128)
+    rc = _load().orc_reduce(C.c_int32(n), _dp(Hb.view(np.float64)), C.c_int32(n), _dp(Sb.view(np.float64)), C.c_int32(n),
+                            _dp(Kb.view(np.float64)), C.c_int32(n))
+    if rc != 0:
+        raise np.linalg.LinAlgError("oracle.reduce_to_standard: S is not positive definite (pivot %d)" % rc)
+    return Kb.T.copy()
+
+
+def jacobi_eigh(K):
+    """(w ascending, Z) of a Hermitian K by the classical cyclic Jacobi method in long double."""
+    K = np.asarray(K, dtype=np.complex128)
+    n = K.shape[0]
+    Kb = _cm(K)
+    w = np.zeros(n, dtype=np.float64)
+    Zb = np.zeros((n, n), dtype=np.complex128)
+    rc = _load().orc_jacobi(C.c_int32(n), _dp(Kb.view(np.float64)), C.c_int32(n), _dp(w), _dp(Zb.view(np.float64)), C.c_int32(n))
+    assert 0 <= rc < 60, "oracle.jacobi_eigh did not converge"
+    return w, Zb.T.copy()
+
+
+def backsolve(L, Z):
+    """C = L^-H Z (eq. 1: Z = L^H X) by back substitution."""
+    L = np.asarray(L, dtype=np.complex128)
+    Z = np.asarray(Z, dtype=np.complex128)
+    n, m = Z.shape
+    Lb, Zb = _cm(L), _cm(Z)
+    Cb = np.zeros((m, n), dtype=np.complex128)
+    rc = _load().orc_backsolve(C.c_int32(n), C.c_int32(m), _dp(Lb.view(np.float64)), C.c_int32(n),
+                               _dp(Zb.view(np.float64)), C.c_int32(n), _dp(Cb.view(np.float64)), C.c_int32(n))
+    assert rc == 0
+    return Cb.T.copy()
+
+
+def subspace_eig(H, S, m=None, solver="jacobi", return_factors=False):
+    """Generalized Hermitian eigen-solve H x = lambda S x by the paper's route (eq. 1):
+    S = L L^H, K = L^-1 H L^-H (two triangular substitutions instead of ZHEGST), K Z = Z Lambda, X = L^-H Z.
+    -> (lambda[m] ascending, C[n, m]) with C^H S C = I (and L, K if return_factors).
+    solver="jacobi": everything in the C oracle in long double (cyclic Jacobi for the standard problem).
+    solver="heevd":  Cholesky, the two substitutions and the back substitution in the C oracle; the standard
+    problem by the library routine the paper names there, "(P)ZHEEVD" = numpy.linalg.eigh.
+    Used where the O(n^3 * sweeps) Jacobi loop is too slow (n > ~300)."""
+    H = np.asarray(H, dtype=np.complex128)
+    S = np.asarray(S, dtype=np.complex128)
+    n = H.shape[0]
+    m = n if m is None else int(m)
+    if solver == "jacobi":
+        Hb, Sb = _cm(H), _cm(S)
+        lam = np.zeros(m, dtype=np.float64)
+        Cb = np.zeros((m, n), dtype=np.complex128)
+        Lb = np.zeros((n, n), dtype=np.complex128)
+        Kb = np.zeros((n, n), dtype=np.complex128)
+        rc = _load().orc_subspace_eig(C.c_int32(n), _dp(Hb.view(np.float64)), C.c_int32(n), _dp(Sb.view(np.float64)), C.c_int32(n),
+                                      C.c_int32(m), _dp(lam), _dp(Cb.view(np.float64)), C.c_int32(n),
+                                      _dp(Lb.view(np.float64)), _dp(Kb.view(np.float64)), C.c_int32(n))
+        if rc != 0:
+            raise np.linalg.LinAlgError("oracle.subspace_eig: S is not positive definite (pivot %d)" % rc)
+        Cm, L, K = Cb.T.copy(), Lb.T.copy(), Kb.T.copy()
+    elif solver == "heevd":
+        L = potrf(S)
+        K = reduce_to_standard(H, S)
+        w, Z = np.linalg.eigh(0.5 * (K + K.conj().T))
+        lam = w[:m].copy()
+        Cm = backsolve(L, Z[:, :m])
+    else:
+        raise ValueError(solver)
+    return (lam, Cm, L, K) if return_factors else (lam, Cm)
+
+
+def rotate2(Y, HY, Cmat, lam):
+    """Rayleigh-Ritz update with residual (Knyazev's LOBPCG, cited PAPER.md:19,124):
+        X'[j] = sum_c Y[c] C[c, j],   HX'[j] = sum_c HY[c] C[c, j],   R[j] = HX'[j] - lam[j] X'[j]
+    for Y, HY [n, Ng] (row = one column of the block), Cmat n x m, lam[m] real.  Three plain products/loops in
+    long double, rounded to double once at the end."""
+    Yl = np.asarray(Y, dtype=np.complex128).astype(np.clongdouble)
+    HYl = np.asarray(HY, dtype=np.complex128).astype(np.clongdouble)
+    Cl = np.asarray(Cmat, dtype=np.complex128).astype(np.clongdouble)
+    X = Cl.T @ Yl
+    HX = Cl.T @ HYl
+    R = HX - np.asarray(lam, dtype=np.longdouble)[:, None] * X
+    return X.astype(np.complex128), HX.astype(np.complex128), R.astype(np.complex128)
