@@ -14,9 +14,15 @@
  * a message.  "device" pointers are CUDA device pointers of the current device, which must be
  * the device the plan was created on (INVALID_ARG otherwise); "host" pointers are ordinary
  * host memory.  `stream` is a cudaStream_t passed as void* (NULL =
- * the legacy default stream).  The compute calls are asynchronous on `stream` and never
- * synchronise with the host; a plan owns one workspace, so at most one call per plan may
- * be in flight at a time (calls on the same stream are naturally ordered).
+ * the legacy default stream).  rsdft_apply_h, rsdft_subspace_gram, rsdft_subspace_rotate and
+ * rsdft_subspace_rotate2 are asynchronous on `stream`; the first call with a new shape may
+ * allocate plan-owned workspace (cudaMalloc, which can synchronise the device), steady-state
+ * calls neither allocate nor synchronise.  rsdft_subspace_eig and rsdft_block_step_host
+ * synchronise with the host (documented at each).  A plan owns one workspace, so at most one
+ * call per plan may be in flight at a time (calls on the same stream are naturally ordered).
+ * Work the caller queues on OTHER streams (e.g. rsdft_plan_set_vloc on stream A, then
+ * rsdft_apply_h on stream B) must be ordered by the caller; rsdft_block_step_host, which runs
+ * on plan-owned streams, orders itself after the last rsdft_plan_set_vloc.
  */
 #ifndef RSDFT_H
 #define RSDFT_H
@@ -32,7 +38,9 @@ typedef enum {
     RSDFT_INVALID_ARG = -1, /* null pointer, ncol <= 0, ld < Ng, X aliases HX, |m| > l, l > 2, ... */
     RSDFT_UNSUPPORTED = -2, /* grid length outside {16,...,128 step 16, 160, 192, 256}; box <= 0; 2*rc >= min L */
     RSDFT_ALLOC = -3,       /* host or device allocation failed */
-    RSDFT_CUDA = -4         /* CUDA runtime error; message carries cudaGetErrorString */
+    RSDFT_CUDA = -4,        /* CUDA runtime error; message carries cudaGetErrorString */
+    RSDFT_NOT_POSITIVE_DEFINITE = -5, /* rsdft_subspace_eig: the Cholesky factorisation of S_sub met a pivot <= 0 */
+    RSDFT_NO_CONVERGENCE = -6         /* rsdft_subspace_eig: the eigen-solver did not converge */
 } rsdft_status;
 
 typedef struct rsdft_plan rsdft_plan_t; /* opaque, library-owned */
@@ -126,6 +134,48 @@ int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ld
 int rsdft_subspace_rotate(rsdft_plan_t *plan, int32_t n, int32_t m, const void *Y, int64_t ldy,
                           const void *C, int32_t ldc, void *Out, int64_t ldo, void *stream);
 
+/* Rayleigh-Ritz update with the LOBPCG residual fused in (Knyazev's method as cited by
+ * PAPER.md:19,124): one pass over Y and HY that shares every tile of C between the two products,
+ *   X'[r, j] = sum_c Y[r, c] C[c, j],   HX'[r, j] = sum_c HY[r, c] C[c, j],   R[r, j] = HX'[r, j] - lambda[j] X'[r, j],
+ * j < m.  Y, HY: DEVICE complex128 blocks of n columns (ldy, ldhy >= Ng); C: DEVICE n x m column-major
+ * (ldc >= n); lambda: DEVICE double[m] (the Ritz values rsdft_subspace_eig returns; may be NULL iff R is NULL);
+ * Xout, HXout, R: DEVICE blocks of m columns (ld >= Ng), any of them may be NULL to skip it, none may overlap
+ * Y, HY or each other.  P' = [W, P] C_P is the same call on the sub-block pointers with HY/HXout/R unused
+ * (or rsdft_subspace_rotate).  Asynchronous on `stream`.  Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+int rsdft_subspace_rotate2(rsdft_plan_t *plan, int32_t n, int32_t m, const void *Y, int64_t ldy,
+                           const void *HY, int64_t ldhy, const void *C, int32_t ldc, const double *lambda,
+                           void *Xout, int64_t ldx, void *HXout, int64_t ldhx, void *R, int64_t ldr,
+                           void *stream);
+
+/* Generalized Hermitian eigen-solve of the subspace pencil, H_sub x = lambda S_sub x, by the paper's route
+ * (eq. 1), entirely on the device:
+ *   S = L L^H (blocked Cholesky);  K = L^-1 H L^-H by TWO blocked triangular solves ("two calls to (P)ZTRSM"
+ *   instead of (P)ZHEGST);  K Z = Z Lambda (block Jacobi on the FP64 tensor pipe);  X = L^-H Z.
+ * H_sub, S_sub: DEVICE n x n complex128 column-major (lds >= n), as rsdft_subspace_gram writes them; S_sub's
+ * LOWER triangle is read, H_sub is read in full.  Outputs: lambda DEVICE double[m], the m lowest eigenvalues in
+ * ascending order; C DEVICE n x m column-major (ldc >= n), column j = eigenvector j, normalised C^H S_sub C = I
+ * (phases, and bases inside degenerate eigenspaces, are not unique).  1 <= m <= n <= 16384.
+ * Runs on `stream` and SYNCHRONISES it with the host (once after the Cholesky for the definiteness check, once
+ * per Jacobi sweep for the convergence test); on return the outputs are complete.
+ * Errors: INVALID_ARG, ALLOC, CUDA, NOT_POSITIVE_DEFINITE, NO_CONVERGENCE. */
+int rsdft_subspace_eig(rsdft_plan_t *plan, int32_t n, const void *H_sub, const void *S_sub, int32_t lds,
+                       int32_t m, double *lambda, void *C, int32_t ldc, void *stream);
+
+/* Intermediate results of the last successful rsdft_subspace_eig on this plan (both are unique, so tests compare
+ * them element by element): what = 0: the Cholesky factor L (lower, strict upper part zero); what = 1: the
+ * standard-form matrix K = L^-1 H L^-H.  out: DEVICE n x n complex128 column-major, ld >= n.  Asynchronous. */
+int rsdft_subspace_eig_get(rsdft_plan_t *plan, int32_t what, void *out, int32_t ld, void *stream);
+
+/* Knobs of rsdft_subspace_eig.  reduction 0 (default): K by two triangular solves, the paper's proposal;
+ * 1: the blocked two-sided reduction ZHEGST performs (LAPACK's algorithm, itype 1 lower, on the same kernels),
+ * kept so that the paper's TRSM-vs-HEGST comparison can be measured.  inner_sweeps: Jacobi sweeps
+ * of each 64 x 64 sub-problem per visit (0 = library default 1, at most 16).  Results agree within round-off. */
+int rsdft_plan_set_eig_mode(rsdft_plan_t *plan, int32_t reduction, int32_t inner_sweeps);
+
+/* Timing/diagnostics of the last rsdft_subspace_eig: out[0..7] = {Jacobi sweeps, ms Cholesky, ms reduction to
+ * standard form, ms eigen-solver, ms back substitution, final off(K)/||K||_F, reduction mode, 0}. */
+int rsdft_subspace_eig_stats(const rsdft_plan_t *plan, double *out8);
+
 /* One whole block step with HOST buffers (the end-to-end entry point): copies Y (host, pinned
  * recommended) to the device in panels of 96 columns; each panel goes through rsdft_apply_h as soon as
  * it has arrived and then every [S|H] tile that has become computable is contracted, so both H Y and the
@@ -144,7 +194,7 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
 int rsdft_plan_info(const rsdft_plan_t *plan, int64_t *out8);
 
 /* Tuning knob: number of columns apply_h pushes through its kernel sequence at a time
- * (0 = library default: about 400 MB of orbitals per launch). */
+ * (0 = library default: about 270 MB of orbitals per launch). */
 int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols);
 
 /* Tuning knob: apply_h deals its column batches round-robin to `nstreams` plan-owned CUDA streams
@@ -161,6 +211,11 @@ int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams);
  * anyway): 30 % fewer flops, H_sub exactly Hermitian, equal to mode 0 within round-off.
  * Errors: INVALID_ARG. */
 int rsdft_plan_set_gram_mode(rsdft_plan_t *plan, int32_t h_upper_only);
+
+/* Frees the plan-owned workspaces that grow with the problem (the device copies of Y and HY that
+ * rsdft_block_step_host keeps, the Gram and projector work buffers, the eigen-solver buffers); they are
+ * re-created on the next call that needs them.  Synchronises the device.  Errors: INVALID_ARG, CUDA. */
+int rsdft_plan_release_workspace(rsdft_plan_t *plan);
 
 /* Destroys the plan and frees everything it owns (synchronises the device first). */
 int rsdft_plan_destroy(rsdft_plan_t *plan);

@@ -1,0 +1,530 @@
+// Generalized Hermitian eigen-solve of the LOBPCG subspace pencil by the paper's route (eq. 1;
+// SURVEY 8(f) NEXT-1):   S = L L^H,   K = L^-1 H L^-H  ("two calls to (P)ZTRSM" instead of (P)ZHEGST),
+// K Z = Z Lambda,   X = L^-H Z.   n <= a few thousand, everything on the device, no cuSolver / cuBLAS.
+//
+// Building blocks (all complex128, column-major, element (i, j) at i + j*ld):
+//   zgemm_kernel<TA,TB>      C = alpha op(A) op(B) + beta C on the FP64 tensor pipe (mma.m8n8k4.f64 = DMMA.8x8x4,
+//                            the only native FP64 MMA shape of sm_100a), 64 x 64 tile, register-prefetched K chunks.
+//                            Blocked Cholesky (panel + trailing update), both blocked triangular solves and the
+//                            back substitution are sequences of these with inverted 64 x 64 diagonal blocks.
+//   potf2_trtri_kernel       one CTA: unblocked Cholesky of a 64 x 64 diagonal block in shared memory + its inverse.
+//   conj_transpose_kernel    B = A^H (the second solve K L^H = Z is run as L K^H = Z^H).
+//   Hermitian eigen-solver:  two-sided BLOCK JACOBI.  The matrix is cut into blocks of 32 columns; a round pairs the
+//                            blocks (round-robin tournament: nblk-1 rounds visit every pair once = one sweep);
+//                            jacobi_subeig_kernel diagonalises each pair's 64 x 64 Hermitian sub-matrix in shared
+//                            memory (parallel-ordered 2 x 2 rotations) and returns its unitary J; the update
+//                            K <- Jt^H K Jt, V <- V Jt (Jt = all pairs of the round) is three DMMA products
+//                            (jacobi_colupdate_kernel; the row update is a column update of the conjugate transpose).
+//                            Chosen over Householder tridiagonalisation + QL/D&C because every O(n^3) part is a
+//                            tensor-core product and the method is unconditionally accurate.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "async_copy.cuh"
+
+namespace rsdft {
+
+__device__ __forceinline__ void eig_dmma884(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+constexpr int EIG_NB = 64;        // block size of the Cholesky / triangular solves, and the Jacobi pair dimension
+constexpr int EIG_JB = 32;        // Jacobi block width (a pair is 2 * EIG_JB = 64 columns)
+
+// ------------------------------------------------------------------------------------------------------------
+// C (M x N) = alpha * op(A) * op(B) + beta * C.
+// TA == false: A is M x K, element (m, k) at m + k*lda;  TA == true: op(A) = A^H with A stored K x M.
+// TB == false: B is K x N, element (k, n) at k + n*ldb;  TB == true: op(B) = B^H with B stored N x K.
+// lower != 0 skips the 64 x 64 tiles that lie strictly above the diagonal (square C, trailing updates).
+struct ZgemmArgs {
+    const double2 *A, *B;
+    double2 *C;
+    int64_t lda, ldb, ldc;
+    int32_t M, N, K;
+    double alpha, beta;
+    int32_t lower;
+};
+
+template <bool TA, bool TB>
+__global__ void __launch_bounds__(256) zgemm_kernel(ZgemmArgs a)
+{
+    constexpr int TM = 64, TN = 64, KC = 16, P = KC + 4;      // pitch % 8 == 4: conflict-free LDS.128 fragments
+    __shared__ double2 As[TM * P], Bs[TN * P];
+    const int m0 = blockIdx.x * TM, n0 = blockIdx.y * TN;
+    if (a.lower && n0 >= m0 + TM) return;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp >> 2, wn = warp & 3;                   // 2 x 4 warps, each 32 rows x 16 columns
+    const int g = lane >> 2, t = lane & 3;
+    double cre[4][2][2], cim[4][2][2];
+#pragma unroll
+    for (int x = 0; x < 4; ++x)
+#pragma unroll
+        for (int y = 0; y < 2; ++y) { cre[x][y][0] = cre[x][y][1] = cim[x][y][0] = cim[x][y][1] = 0.0; }
+    double2 ra[4], rb[4];
+    auto fetch = [&](int k0) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int e = tid + i * 256;
+            int m, k;
+            if (TA) { k = e % KC; m = e / KC; } else { m = e % TM; k = e / TM; }
+            double2 v = make_double2(0.0, 0.0);
+            if (m0 + m < a.M && k0 + k < a.K) {
+                v = TA ? a.A[(int64_t)(m0 + m) * a.lda + k0 + k] : a.A[(int64_t)(k0 + k) * a.lda + m0 + m];
+                if (TA) v.y = -v.y;
+            }
+            ra[i] = v;
+            int n, kb;
+            if (TB) { n = e % TN; kb = e / TN; } else { kb = e % KC; n = e / KC; }
+            double2 w = make_double2(0.0, 0.0);
+            if (n0 + n < a.N && k0 + kb < a.K) {
+                w = TB ? a.B[(int64_t)(k0 + kb) * a.ldb + n0 + n] : a.B[(int64_t)(n0 + n) * a.ldb + k0 + kb];
+                if (TB) w.y = -w.y;
+            }
+            rb[i] = w;
+        }
+    };
+    auto stash = [&]() {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int e = tid + i * 256;
+            int m, k;
+            if (TA) { k = e % KC; m = e / KC; } else { m = e % TM; k = e / TM; }
+            As[m * P + k] = ra[i];
+            int n, kb;
+            if (TB) { n = e % TN; kb = e / TN; } else { kb = e % KC; n = e / KC; }
+            Bs[n * P + kb] = rb[i];
+        }
+    };
+    fetch(0);
+    for (int k0 = 0; k0 < a.K; k0 += KC) {
+        __syncthreads();                    // everyone is done with the previous chunk
+        stash();
+        __syncthreads();
+        if (k0 + KC < a.K) fetch(k0 + KC);  // next chunk's global loads fly during the MMAs
+        const double2 *Ap = As + (wm * 32 + g) * P + t;
+        const double2 *Bp = Bs + (wn * 16 + g) * P + t;
+#pragma unroll
+        for (int kk = 0; kk < KC; kk += 4) {
+            double br[2], bi[2];
+#pragma unroll
+            for (int y = 0; y < 2; ++y) { const double2 v = Bp[y * 8 * P + kk]; br[y] = v.x; bi[y] = v.y; }
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                const double2 v = Ap[x * 8 * P + kk];
+                const double ar = v.x, ai = v.y, nai = -v.y;
+#pragma unroll
+                for (int y = 0; y < 2; ++y) {
+                    eig_dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
+                    eig_dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
+                }
+#pragma unroll
+                for (int y = 0; y < 2; ++y) {
+                    eig_dmma884(cre[x][y][0], cre[x][y][1], nai, bi[y]);
+                    eig_dmma884(cim[x][y][0], cim[x][y][1], ai, br[y]);
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int x = 0; x < 4; ++x)
+#pragma unroll
+        for (int y = 0; y < 2; ++y)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int row = m0 + wm * 32 + x * 8 + g, col = n0 + wn * 16 + y * 8 + 2 * t + e;
+                if (row >= a.M || col >= a.N) continue;
+                double2 *c = a.C + (int64_t)col * a.ldc + row;
+                double re = a.alpha * cre[x][y][e], im = a.alpha * cim[x][y][e];
+                if (a.beta != 0.0) { const double2 o = *c; re = fma(a.beta, o.x, re); im = fma(a.beta, o.y, im); }
+                *c = make_double2(re, im);
+            }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Diagonal block k of the blocked Cholesky: reads the nb x nb block at W + k0 + k0*ld (lower triangle, already
+// updated by the trailing products), factors it (unblocked, right-looking, in shared memory), writes L_kk back
+// (upper part zeroed) and its inverse L_kk^-1 into Dinv (64 x 64, lower, zero padded).  info[0] receives
+// k0 + j + 1 for the first non-positive pivot (0 = none).
+__global__ void __launch_bounds__(256) potf2_trtri_kernel(double2 *W, int64_t ld, int k0, int nb, double2 *Dinv, int *info)
+{
+    constexpr int NB = EIG_NB, P = NB + 1;
+    extern __shared__ __align__(16) unsigned char eig_smem_raw[];
+    double2 *A = reinterpret_cast<double2 *>(eig_smem_raw);   // [NB][P]  A[i*P + j] = element (i, j)
+    double2 *X = A + NB * P;                                   // inverse
+    __shared__ int bad;
+    const int tid = threadIdx.x;
+    if (tid == 0) bad = 0;
+    for (int e = tid; e < NB * NB; e += 256) {
+        const int i = e % NB, j = e / NB;
+        double2 v = make_double2(i == j ? 1.0 : 0.0, 0.0);      // identity padding beyond nb
+        if (i < nb && j < nb) v = (i >= j) ? W[(int64_t)(k0 + j) * ld + k0 + i] : make_double2(0.0, 0.0);
+        A[i * P + j] = v;
+    }
+    __syncthreads();
+    for (int j = 0; j < NB; ++j) {
+        const double d = A[j * P + j].x;
+        if (!(d > 0.0)) { if (tid == 0 && !bad) bad = k0 + j + 1; }
+        const double inv = 1.0 / sqrt(d > 0.0 ? d : 1.0);
+        __syncthreads();
+        if (tid == 0) A[j * P + j] = make_double2(sqrt(d > 0.0 ? d : 1.0), 0.0);
+        for (int i = j + 1 + tid; i < NB; i += 256) { double2 v = A[i * P + j]; v.x *= inv; v.y *= inv; A[i * P + j] = v; }
+        __syncthreads();
+        // trailing update of the lower triangle: A[i][k] -= A[i][j] * conj(A[k][j]),  j < k <= i
+        const int rem = NB - 1 - j;
+        for (int e = tid; e < rem * rem; e += 256) {
+            const int i = j + 1 + e / rem, k = j + 1 + e % rem;
+            if (k > i) continue;
+            const double2 x = A[i * P + j], y = A[k * P + j];
+            double2 v = A[i * P + k];
+            v.x -= x.x * y.x + x.y * y.y;
+            v.y -= x.y * y.x - x.x * y.y;
+            A[i * P + k] = v;
+        }
+        __syncthreads();
+    }
+    // inverse of the lower-triangular factor, one column per thread: L x = e_j by forward substitution
+    if (tid < NB) {
+        const int j = tid;
+        for (int i = 0; i < NB; ++i) {
+            double sr = (i == j) ? 1.0 : 0.0, si = 0.0;
+            for (int k = j; k < i; ++k) {
+                const double2 l = A[i * P + k], x = X[k * P + j];
+                sr -= l.x * x.x - l.y * x.y;
+                si -= l.x * x.y + l.y * x.x;
+            }
+            const double dinv = 1.0 / A[i * P + i].x;
+            X[i * P + j] = (i < j) ? make_double2(0.0, 0.0) : make_double2(sr * dinv, si * dinv);
+        }
+    }
+    __syncthreads();
+    for (int e = tid; e < NB * NB; e += 256) {
+        const int i = e % NB, j = e / NB;
+        if (i < nb && j < nb) W[(int64_t)(k0 + j) * ld + k0 + i] = A[i * P + j];
+        Dinv[j * NB + i] = (i < nb && j < nb) ? X[i * P + j] : make_double2(0.0, 0.0);
+    }
+    if (tid == 0 && bad) atomicCAS(info, 0, bad);
+}
+
+// B (cols x rows, ldb) = A^H for A (rows x cols, lda); 32 x 32 tiles through shared memory.
+__global__ void __launch_bounds__(256) conj_transpose_kernel(const double2 *A, int64_t lda, double2 *B, int64_t ldb, int rows, int cols)
+{
+    __shared__ double2 tile[32][33];
+    const int i0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+    for (int e = threadIdx.x; e < 1024; e += 256) {
+        const int i = e & 31, j = e >> 5;
+        if (i0 + i < rows && j0 + j < cols) tile[j][i] = A[(int64_t)(j0 + j) * lda + i0 + i];
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < 1024; e += 256) {
+        const int j = e & 31, i = e >> 5;
+        if (i0 + i < rows && j0 + j < cols) { const double2 v = tile[j][i]; B[(int64_t)(i0 + i) * ldb + j0 + j] = make_double2(v.x, -v.y); }
+    }
+}
+
+// rows x cols copy between column-major matrices; mode 1 zeroes the strict upper triangle (L for the caller),
+// mode 2 copies the strict upper triangle only
+__global__ void __launch_bounds__(256) mat_copy_kernel(const double2 *A, int64_t lda, double2 *B, int64_t ldb, int rows, int cols, int mode)
+{
+    const int64_t total = (int64_t)rows * cols;
+    for (int64_t e = blockIdx.x * 256ll + threadIdx.x; e < total; e += (int64_t)gridDim.x * 256) {
+        const int i = (int)(e % rows), j = (int)(e / rows);
+        if (mode == 2 && i >= j) continue;
+        double2 v = A[(int64_t)j * lda + i];
+        if (mode == 1 && i < j) v = make_double2(0.0, 0.0);
+        B[(int64_t)j * ldb + i] = v;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Block Jacobi.  Kp / V are npad x npad (npad a multiple of 64).
+
+// Kp = (K + K^H)/2 on the leading n x n (real diagonal), `big` on the padded diagonal, 0 elsewhere; V = I;
+// part[b] = sum over this CTA's elements of |K_ij|^2 (fixed order inside the CTA).
+__global__ void __launch_bounds__(256) jacobi_prepare_kernel(const double2 *K, int64_t ldk, int n, int npad, double2 *Kp, double2 *V, double *part)
+{
+    __shared__ double red[256];
+    double acc = 0.0;
+    const int64_t total = (int64_t)npad * npad;
+    for (int64_t e = blockIdx.x * 256ll + threadIdx.x; e < total; e += (int64_t)gridDim.x * 256) {
+        const int i = (int)(e % npad), j = (int)(e / npad);
+        double2 v = make_double2(0.0, 0.0);
+        if (i < n && j < n) {
+            const double2 x = K[(int64_t)j * ldk + i], y = K[(int64_t)i * ldk + j];
+            v = make_double2(0.5 * (x.x + y.x), i == j ? 0.0 : 0.5 * (x.y - y.y));
+            acc += v.x * v.x + v.y * v.y;
+        }
+        Kp[e] = v;
+        V[e] = make_double2(i == j ? 1.0 : 0.0, 0.0);
+    }
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) { if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s]; __syncthreads(); }
+    if (threadIdx.x == 0) part[blockIdx.x] = red[0];
+}
+
+// the padded diagonal gets a value above every eigenvalue so that padded "eigenvalues" sort last and never rotate
+__global__ void jacobi_pad_diag_kernel(double2 *Kp, int n, int npad, const double *norm2)
+{
+    const int i = n + blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < npad) Kp[(int64_t)i * npad + i] = make_double2(4.0 * sqrt(norm2[0]) + 1.0, 0.0);
+}
+
+// out[0] = sum of part[0..np) in index order (deterministic)
+__global__ void sum_partials_kernel(const double *part, int np, double *out)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double s = 0.0;
+        for (int i = 0; i < np; ++i) s += part[i];
+        out[0] = s;
+    }
+}
+
+// part[b] = sum_{i != j, both < n} |Kp_ij|^2 over this CTA's elements
+__global__ void __launch_bounds__(256) jacobi_offnorm_kernel(const double2 *Kp, int n, int npad, double *part)
+{
+    __shared__ double red[256];
+    double acc = 0.0;
+    const int64_t total = (int64_t)n * n;
+    for (int64_t e = blockIdx.x * 256ll + threadIdx.x; e < total; e += (int64_t)gridDim.x * 256) {
+        const int i = (int)(e % n), j = (int)(e / n);
+        if (i != j) { const double2 v = Kp[(int64_t)j * npad + i]; acc += v.x * v.x + v.y * v.y; }
+    }
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) { if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s]; __syncthreads(); }
+    if (threadIdx.x == 0) part[blockIdx.x] = red[0];
+}
+
+// One CTA per block pair (p, q) of the round: load the 64 x 64 Hermitian sub-matrix
+//   [ K_pp K_pq ; K_qp K_qq ]  (symmetrised from both triangles), run up to `inner` sweeps of parallel-ordered
+// 2 x 2 Jacobi rotations in shared memory (63 steps of 32 disjoint index pairs per sweep, circle method), and
+// write the accumulated unitary J (64 x 64, column-major) to Jbuf[pair].  For a_ij = r e^{i phi}:
+//   tau = (a_jj - a_ii)/(2r), t = sign(tau)/(|tau| + sqrt(1 + tau^2)), c = 1/sqrt(1 + t^2), s = t c,
+//   J = [[c, s], [-s e^{-i phi}, c e^{-i phi}]],   A <- J^H A J.
+// A sweep in which no |a_ij| exceeded `tiny` (passed in norm2[1] = absolute threshold) ends the loop early.
+// cross != 0: only the 32 x 32 index pairs (i in block p, j in block q) are rotated (32 steps of 32 disjoint pairs):
+// over the nblk-1 rounds of a sweep every off-diagonal element is then annihilated exactly once (cyclic Jacobi in
+// a block round-robin ordering); the first round of each sweep runs with cross == 0 and also covers the pairs
+// inside the two diagonal blocks (63 steps).
+__global__ void __launch_bounds__(256) jacobi_subeig_kernel(const double2 *Kp, int npad, const int2 *pairs, double2 *Jbuf,
+                                                            int inner, const double *norm2, int cross)
+{
+    constexpr int D = 2 * EIG_JB, P = D + 1;
+    extern __shared__ __align__(16) unsigned char eig_smem_raw[];
+    double2 *A = reinterpret_cast<double2 *>(eig_smem_raw);   // [D][P]
+    double2 *V = A + D * P;
+    __shared__ double rc[32], rs[32], rer[32], rei[32];
+    __shared__ int ri[32], rj[32];
+    __shared__ int active;
+    const int tid = threadIdx.x;
+    const int2 pq = pairs[blockIdx.x];
+    const double tiny = norm2[1];
+    auto gidx = [&](int a) { return a < EIG_JB ? pq.x * EIG_JB + a : pq.y * EIG_JB + a - EIG_JB; };
+    for (int e = tid; e < D * D; e += 256) {
+        const int i = e % D, j = e / D;
+        const int gi = gidx(i), gj = gidx(j);
+        const double2 x = Kp[(int64_t)gj * npad + gi], y = Kp[(int64_t)gi * npad + gj];
+        A[i * P + j] = make_double2(0.5 * (x.x + y.x), i == j ? 0.0 : 0.5 * (x.y - y.y));
+        V[i * P + j] = make_double2(i == j ? 1.0 : 0.0, 0.0);
+    }
+    __syncthreads();
+    for (int sweep = 0; sweep < inner; ++sweep) {
+        if (tid == 0) active = 0;
+        __syncthreads();
+        const int nsteps = cross ? EIG_JB : D - 1;
+        for (int step = 0; step < nsteps; ++step) {
+            if (tid < 32) {
+                int i, j;
+                if (cross) { i = tid; j = EIG_JB + ((tid + step) & (EIG_JB - 1)); }
+                else if (tid == 0) { i = D - 1; j = step; }
+                else { i = (step + tid) % (D - 1); j = (step - tid + (D - 1)) % (D - 1); }
+                if (i > j) { const int s = i; i = j; j = s; }
+                const double2 aij = A[i * P + j];
+                const double r = sqrt(aij.x * aij.x + aij.y * aij.y);
+                double c = 1.0, s = 0.0, er = 1.0, ei = 0.0;
+                if (r > tiny) {
+                    const double tau = (A[j * P + j].x - A[i * P + i].x) / (2.0 * r);
+                    const double tt = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+                    c = 1.0 / sqrt(1.0 + tt * tt);
+                    s = tt * c;
+                    er = aij.x / r; ei = -aij.y / r;             // e^{-i phi}
+                    active = 1;
+                }
+                rc[tid] = c; rs[tid] = s; rer[tid] = er; rei[tid] = ei; ri[tid] = i; rj[tid] = j;
+            }
+            __syncthreads();
+            // columns: A <- A J, V <- V J   (lanes run over rows: pitch 65 is conflict-free)
+            for (int item = tid; item < D * 32; item += 256) {
+                const int row = item % D, k = item / D;
+                const int i = ri[k], j = rj[k];
+                const double c = rc[k], s = rs[k], er = rer[k], ei = rei[k];
+                // J_ii = c, J_ij = s, J_ji = -s e, J_jj = c e   (e = e^{-i phi})
+                {
+                    const double2 x = A[row * P + i], y = A[row * P + j];
+                    const double yer = y.x * er - y.y * ei, yei = y.x * ei + y.y * er;   // y * e
+                    A[row * P + i] = make_double2(c * x.x - s * yer, c * x.y - s * yei);
+                    A[row * P + j] = make_double2(s * x.x + c * yer, s * x.y + c * yei);
+                }
+                {
+                    const double2 x = V[row * P + i], y = V[row * P + j];
+                    const double yer = y.x * er - y.y * ei, yei = y.x * ei + y.y * er;
+                    V[row * P + i] = make_double2(c * x.x - s * yer, c * x.y - s * yei);
+                    V[row * P + j] = make_double2(s * x.x + c * yer, s * x.y + c * yei);
+                }
+            }
+            __syncthreads();
+            // rows: A <- J^H A   (lanes run over columns)
+            for (int item = tid; item < D * 32; item += 256) {
+                const int col = item % D, k = item / D;
+                const int i = ri[k], j = rj[k];
+                const double c = rc[k], s = rs[k], er = rer[k], ei = rei[k];
+                const double2 x = A[i * P + col], y = A[j * P + col];
+                const double ycr = y.x * er + y.y * ei, yci = y.y * er - y.x * ei;       // y * conj(e)
+                A[i * P + col] = make_double2(c * x.x - s * ycr, c * x.y - s * yci);
+                A[j * P + col] = make_double2(s * x.x + c * ycr, s * x.y + c * yci);
+            }
+            __syncthreads();
+        }
+        if (!active) break;
+    }
+    double2 *J = Jbuf + (int64_t)blockIdx.x * D * D;
+    for (int e = tid; e < D * D; e += 256) {
+        const int i = e % D, j = e / D;
+        J[e] = V[i * P + j];
+    }
+}
+
+// Out[:, cols(p,q)] = In[:, cols(p,q)] * J_pair for every pair of the round (tr == 0), or the conjugate transpose
+// of that product stored at Out[cols(p,q), :] (tr == 1).  In, Out: npad x npad, Out != In.  Up to two independent
+// (In, Out, tr) sets per launch (blockIdx.z): the V update rides along with the first K update.
+// CTA (pair, g, z) keeps the pair's J (64 x 64) resident in shared memory and walks the 64-row tiles g, g + G, ...;
+// the next tile arrives by cp.async while the current one is multiplied: 8 warps, each 32 rows x 16 columns
+// (4 x 2 DMMA tiles), K = 64.
+struct ColUpdArgs {
+    const double2 *In[2];
+    double2 *Out[2];
+    int32_t tr[2];
+    int32_t npad;
+    const int2 *pairs;
+    const double2 *Jbuf;
+};
+
+__global__ void __launch_bounds__(256, 1) jacobi_colupdate_kernel(ColUpdArgs a)
+{
+    constexpr int D = 2 * EIG_JB, TM = 64, P = D + 4;
+    extern __shared__ __align__(16) unsigned char eig_smem_raw[];
+    double2 *Bs = reinterpret_cast<double2 *>(eig_smem_raw);  // [D][P]      Bs[n*P + k] = J[k][n]
+    double2 *As0 = Bs + D * P;                                 // [2][TM][P]  As[m*P + k]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp >> 2, wn = warp & 3;
+    const int g = lane >> 2, t = lane & 3;
+    const int z = blockIdx.z;
+    const double2 *In = a.In[z];
+    double2 *Out = a.Out[z];
+    const int tr = a.tr[z], npad = a.npad;
+    const int2 pq = a.pairs[blockIdx.x];
+    auto gcol = [&](int c) { return c < EIG_JB ? pq.x * EIG_JB + c : pq.y * EIG_JB + c - EIG_JB; };
+    const double2 *J = a.Jbuf + (int64_t)blockIdx.x * D * D;
+    for (int e = tid; e < D * D; e += 256) {
+        const int k = e % D, n = e / D;
+        cp_async16(Bs + n * P + k, J + e);
+    }
+    const int ntiles = npad / TM;
+    auto issue = [&](int buf, int rt) {
+        double2 *As = As0 + buf * TM * P;
+        const int r0 = rt * TM;
+        for (int e = tid; e < TM * D; e += 256) {
+            const int m = e % TM, k = e / TM;
+            cp_async16(As + m * P + k, In + (int64_t)gcol(k) * npad + r0 + m);
+        }
+    };
+    int rt = blockIdx.y;
+    if (rt < ntiles) issue(0, rt);
+    cp_async_commit();
+    int buf = 0;
+    for (; rt < ntiles; rt += gridDim.y, buf ^= 1) {
+        if (rt + (int)gridDim.y < ntiles) issue(buf ^ 1, rt + gridDim.y);
+        cp_async_commit();
+        cp_async_wait<1>();
+        __syncthreads();
+        double cre[4][2][2], cim[4][2][2];
+#pragma unroll
+        for (int x = 0; x < 4; ++x)
+#pragma unroll
+            for (int y = 0; y < 2; ++y) { cre[x][y][0] = cre[x][y][1] = cim[x][y][0] = cim[x][y][1] = 0.0; }
+        const double2 *Ap = As0 + buf * TM * P + (wm * 32 + g) * P + t;
+        const double2 *Bp = Bs + (wn * 16 + g) * P + t;
+#pragma unroll 4
+        for (int kk = 0; kk < D; kk += 4) {
+            double br[2], bi[2];
+#pragma unroll
+            for (int y = 0; y < 2; ++y) { const double2 v = Bp[y * 8 * P + kk]; br[y] = v.x; bi[y] = v.y; }
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                const double2 v = Ap[x * 8 * P + kk];
+                const double ar = v.x, ai = v.y, nai = -v.y;
+#pragma unroll
+                for (int y = 0; y < 2; ++y) {
+                    eig_dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
+                    eig_dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
+                }
+#pragma unroll
+                for (int y = 0; y < 2; ++y) {
+                    eig_dmma884(cre[x][y][0], cre[x][y][1], nai, bi[y]);
+                    eig_dmma884(cim[x][y][0], cim[x][y][1], ai, br[y]);
+                }
+            }
+        }
+        const int r0 = rt * TM;
+#pragma unroll
+        for (int x = 0; x < 4; ++x)
+#pragma unroll
+            for (int y = 0; y < 2; ++y)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int row = r0 + wm * 32 + x * 8 + g;
+                    const int col = gcol(wn * 16 + y * 8 + 2 * t + e);
+                    if (tr) Out[(int64_t)row * npad + col] = make_double2(cre[x][y][e], -cim[x][y][e]);
+                    else Out[(int64_t)col * npad + row] = make_double2(cre[x][y][e], cim[x][y][e]);
+                }
+        __syncthreads();                  // the buffer just read is the target of the next prefetch
+    }
+    cp_async_wait<0>();
+}
+
+// Eigenvalues = real diagonal of the converged Kp; rank them ascending (ties by index), lambda[rank] = d for
+// rank < m, perm[rank] = i.
+__global__ void __launch_bounds__(256) eig_rank_kernel(const double2 *Kp, int n, int npad, int m, double *lambda, int *perm)
+{
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (i >= n) return;
+    const double d = Kp[(int64_t)i * npad + i].x;
+    int rank = 0;
+    for (int j = 0; j < n; ++j) {
+        const double e = Kp[(int64_t)j * npad + j].x;
+        rank += (e < d) || (e == d && j < i);
+    }
+    perm[rank] = i;
+    if (rank < m) lambda[rank] = d;
+}
+
+// Zs[:, r] = V[0:n, perm[r]] / ||V[0:n, perm[r]]||_2 for r < m: one CTA per selected eigenvector.  The accumulated
+// product of rotations drifts from unit column norm by ~1e-12 over a few hundred updates; the renormalisation
+// (fixed-order reduction) brings Z^H Z = I back to round-off.
+__global__ void __launch_bounds__(256) eig_gather_kernel(const double2 *V, int npad, int n, int m, const int *perm, double2 *Zs, int64_t ldz)
+{
+    __shared__ double red[256];
+    const int r = blockIdx.x;
+    const double2 *src = V + (int64_t)perm[r] * npad;
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n; i += 256) { const double2 v = src[i]; acc += v.x * v.x + v.y * v.y; }
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) { if (threadIdx.x < s) red[threadIdx.x] += red[threadIdx.x + s]; __syncthreads(); }
+    const double inv = 1.0 / sqrt(red[0]);
+    for (int i = threadIdx.x; i < n; i += 256) { const double2 v = src[i]; Zs[(int64_t)r * ldz + i] = make_double2(v.x * inv, v.y * inv); }
+}
+
+}  // namespace rsdft

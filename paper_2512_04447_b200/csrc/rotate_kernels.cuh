@@ -142,4 +142,142 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate_dmma_kernel(RotateArg
             }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Two-output update with the LOBPCG residual fused into the epilogue:
+//   X'[r, j] = sum_c Y[r, c] C[c, j],   HX'[r, j] = sum_c HY[r, c] C[c, j],   R[r, j] = HX'[r, j] - lambda_j X'[r, j].
+// One CTA owns a TM x TN tile of BOTH products: every C stage in shared memory feeds the Y and the HY
+// accumulators, so C is staged once, Y and HY are read once, and the three outputs are written once.
+struct Rotate2Args {
+    const double2 *Y, *HY;  // [n][ldy], [n][ldhy]
+    const double2 *C;       // column-major n x m
+    const double *lambda;   // [m] real Ritz values (may be NULL when R is NULL)
+    double2 *X, *HX, *R;    // [m][ldx], [m][ldhx], [m][ldr]; any may be NULL
+    int64_t ldy, ldhy, ldx, ldhx, ldr, ng;
+    int32_t n, m, ldc, jtiles;
+};
+
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES>
+struct Rotate2Cfg {
+    static constexpr int TM = WGM * FA * 8, TN = WGN * FB * 8;
+    static constexpr int THREADS = WGM * WGN * 32;
+    static constexpr int PA = TM + 2;              // A stages: [KC][PA] for Y and for HY
+    static constexpr int PB = KC + 4;              // B stage: [TN][PB]
+    static constexpr int STAGE_ELEMS = 2 * KC * PA + TN * PB;
+    static constexpr size_t SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(double2);
+};
+
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES>
+__global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate2_dmma_kernel(Rotate2Args a)
+{
+    using Cfg = Rotate2Cfg<WGM, WGN, FA, FB, KC, STAGES>;
+    constexpr int TM = Cfg::TM, TN = Cfg::TN, PA = Cfg::PA, PB = Cfg::PB, NT = Cfg::THREADS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2 *sm = reinterpret_cast<double2 *>(smem_raw);
+
+    const int64_t unit = blockIdx.x;
+    const int64_t rt = unit / a.jtiles;
+    const int jt = (int)(unit - rt * a.jtiles);
+    const int64_t r0 = rt * TM;
+    const int j0 = jt * TN;
+    const int nch = (a.n + KC - 1) / KC;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wm = warp / WGN, wn = warp % WGN;
+    const int g = lane >> 2, t = lane & 3;
+
+    auto load_stage = [&](int stage, int chunk) {
+        double2 *As = sm + (size_t)stage * Cfg::STAGE_ELEMS;
+        double2 *Hs = As + KC * PA;
+        double2 *Bs = Hs + KC * PA;
+        const int c0 = chunk * KC;
+#pragma unroll
+        for (int e = tid; e < KC * TM; e += NT) {
+            const int k = e / TM, r = e - k * TM;
+            if (c0 + k < a.n && r0 + r < a.ng) {
+                cp_async16(As + k * PA + r, a.Y + (int64_t)(c0 + k) * a.ldy + r0 + r);
+                cp_async16(Hs + k * PA + r, a.HY + (int64_t)(c0 + k) * a.ldhy + r0 + r);
+            } else {
+                As[k * PA + r] = make_double2(0.0, 0.0);
+                Hs[k * PA + r] = make_double2(0.0, 0.0);
+            }
+        }
+#pragma unroll
+        for (int e = tid; e < TN * KC; e += NT) {
+            const int j = e / KC, k = e - j * KC;
+            double2 *d = Bs + j * PB + k;
+            if (j0 + j < a.m && c0 + k < a.n) cp_async16(d, a.C + (int64_t)(j0 + j) * a.ldc + c0 + k);
+            else *d = make_double2(0.0, 0.0);
+        }
+    };
+
+    double xre[FA][FB][2], xim[FA][FB][2], hre[FA][FB][2], him[FA][FB][2];
+#pragma unroll
+    for (int x = 0; x < FA; ++x)
+#pragma unroll
+        for (int y = 0; y < FB; ++y)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) { xre[x][y][e] = xim[x][y][e] = hre[x][y][e] = him[x][y][e] = 0.0; }
+
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nch) load_stage(s, s);
+        cp_async_commit();
+    }
+    for (int ch = 0; ch < nch; ++ch) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            const int nx = ch + STAGES - 1;
+            if (nx < nch) load_stage(nx % STAGES, nx);
+            cp_async_commit();
+        }
+        const double2 *As = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + t * PA + wm * FA * 8 + g;
+        const double2 *Hs = As + KC * PA;
+        const double2 *Bs = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + 2 * KC * PA + (wn * FB * 8 + g) * PB + t;
+#pragma unroll
+        for (int kk = 0; kk < KC; kk += 4) {
+            double br[FB], bi[FB];
+#pragma unroll
+            for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PB + kk]; br[y] = v.x; bi[y] = v.y; }
+#pragma unroll
+            for (int x = 0; x < FA; ++x) {
+                const double2 v = As[kk * PA + x * 8];
+                const double2 w = Hs[kk * PA + x * 8];
+#pragma unroll
+                for (int y = 0; y < FB; ++y) {
+                    rot_dmma884(xre[x][y][0], xre[x][y][1], v.x, br[y]);
+                    rot_dmma884(xim[x][y][0], xim[x][y][1], v.x, bi[y]);
+                    rot_dmma884(hre[x][y][0], hre[x][y][1], w.x, br[y]);
+                    rot_dmma884(him[x][y][0], him[x][y][1], w.x, bi[y]);
+                }
+                const double nvy = -v.y, nwy = -w.y;
+#pragma unroll
+                for (int y = 0; y < FB; ++y) {
+                    rot_dmma884(xre[x][y][0], xre[x][y][1], nvy, bi[y]);
+                    rot_dmma884(xim[x][y][0], xim[x][y][1], v.y, br[y]);
+                    rot_dmma884(hre[x][y][0], hre[x][y][1], nwy, bi[y]);
+                    rot_dmma884(him[x][y][0], him[x][y][1], w.y, br[y]);
+                }
+            }
+        }
+    }
+    cp_async_wait<0>();
+
+#pragma unroll
+    for (int y = 0; y < FB; ++y)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int j = j0 + (wn * FB + y) * 8 + 2 * t + e;
+            if (j >= a.m) continue;
+            const double lam = a.R ? a.lambda[j] : 0.0;
+#pragma unroll
+            for (int x = 0; x < FA; ++x) {
+                const int64_t r = r0 + (wm * FA + x) * 8 + g;
+                if (r >= a.ng) continue;
+                if (a.X) a.X[(int64_t)j * a.ldx + r] = make_double2(xre[x][y][e], xim[x][y][e]);
+                if (a.HX) a.HX[(int64_t)j * a.ldhx + r] = make_double2(hre[x][y][e], him[x][y][e]);
+                if (a.R) a.R[(int64_t)j * a.ldr + r] = make_double2(fma(-lam, xre[x][y][e], hre[x][y][e]), fma(-lam, xim[x][y][e], him[x][y][e]));
+            }
+        }
+}
+
 }  // namespace rsdft

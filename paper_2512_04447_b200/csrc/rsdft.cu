@@ -15,6 +15,7 @@
 #include <string>
 #include <vector>
 
+#include "eig_kernels.cuh"
 #include "fft3_kernels.cuh"
 #include "gram_kernels.cuh"
 #include "nonlocal_kernels.cuh"
@@ -65,6 +66,14 @@ struct DevBuf {
         cudaError_t e = alloc(h.size());
         if (e != cudaSuccess || h.empty()) return e;
         return cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+    }
+    // stream-ordered upload for buffers that kernels on `st` read next: the pageable source is staged
+    // before cudaMemcpyAsync returns, and the copy is ordered before later work on `st`
+    cudaError_t upload_async(const std::vector<T> &h, cudaStream_t st)
+    {
+        cudaError_t e = ensure(h.size());
+        if (e != cudaSuccess || h.empty()) return e;
+        return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st);
     }
     size_t bytes() const { return n * sizeof(T); }
 };
@@ -119,17 +128,33 @@ struct rsdft_plan {
     DevBuf<double2> hostY, hostHY, hostHS;
     cudaStream_t s_copy = nullptr, s_comp = nullptr;
     std::vector<cudaEvent_t> ev;
+    cudaEvent_t ev_vloc = nullptr;                    // recorded by set_vloc on the caller's stream; block_step_host waits on it
+    bool vloc_pending = false;
+
+    // generalized eigen-solve (rsdft_subspace_eig): workspace, created on first use
+    DevBuf<double2> eg_L, eg_B, eg_Z, eg_Dinv, eg_Kp, eg_Tp, eg_V0, eg_V1, eg_J, eg_Zs;
+    DevBuf<double> eg_scal;                           // [0] ||K||_F^2, [1] rotation threshold, [2] off(K)^2, [8..] partial sums
+    DevBuf<int> eg_info, eg_perm;
+    DevBuf<int2> eg_pairs;
+    int eg_pairs_nblk = -1;
+    int eg_n = 0;                                     // size of the last successful solve (rsdft_subspace_eig_get)
+    int eig_mode = 0;                                 // 0: two triangular solves (the paper's route), 1: ZHEGST-style
+    int eig_inner = 1;                                // inner sweeps of the 64 x 64 sub-problems per visit
+    double eig_stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    cudaEvent_t eg_ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
 
     int64_t last_launches = 0;
 
     ~rsdft_plan()
     {
+        for (auto e : eg_ev) if (e) cudaEventDestroy(e);
         for (auto e : ev) cudaEventDestroy(e);
         for (int i = 0; i < MAX_STREAMS; ++i) {
             if (s_batch[i]) cudaStreamDestroy(s_batch[i]);
             if (ev_join[i]) cudaEventDestroy(ev_join[i]);
         }
         if (ev_fork) cudaEventDestroy(ev_fork);
+        if (ev_vloc) cudaEventDestroy(ev_vloc);
         if (s_copy) cudaStreamDestroy(s_copy);
         if (s_comp) cudaStreamDestroy(s_comp);
     }
@@ -139,7 +164,9 @@ struct rsdft_plan {
         for (int a = 0; a < 3; ++a) b += tw[a].bytes();
         b += kin_x.bytes() + kin_yz.bytes() + vloc.bytes() + pt_off.bytes() + beta_off.bytes() + idx.bytes() +
              nproj_a.bytes() + beta.bytes() + Dmat.bytes() + chunks.bytes() + atom_chunk0.bytes() + atom_chunks.bytes() +
-             gram_work.bytes() + gram_tiles.bytes() + gram_panel_tiles.bytes() + hostY.bytes() + hostHY.bytes() + hostHS.bytes();
+             gram_work.bytes() + gram_tiles.bytes() + gram_panel_tiles.bytes() + hostY.bytes() + hostHY.bytes() + hostHS.bytes() +
+             eg_L.bytes() + eg_B.bytes() + eg_Z.bytes() + eg_Dinv.bytes() + eg_Kp.bytes() + eg_Tp.bytes() + eg_V0.bytes() +
+             eg_V1.bytes() + eg_J.bytes() + eg_Zs.bytes();
         for (int i = 0; i < MAX_STREAMS; ++i) b += pp[i].bytes() + pq[i].bytes();
         return b;
     }
@@ -446,12 +473,12 @@ cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 
 template <int MT>
 void launch_project_mt(const SphereTables &t, const double2 *X, int64_t ldx, int ncol, double dV, double2 *pp,
-                       cudaStream_t st)
+                       int sms, cudaStream_t st)
 {
     // widest column group (most beta/idx reuse) that still leaves >= ~8 CTAs of 4 warps per SM: the
     // kernel is latency-bound on its gathers, so warps in flight matter more than reuse
     const int gx = (t.nchunks + 3) / 4;
-    const int64_t want = 148 * 8;
+    const int64_t want = (int64_t)sms * 8;
     if (ncol > 16 && (int64_t)gx * ((ncol + 31) / 32) >= want)
         project_kernel<MT, 4><<<dim3(gx, (ncol + 31) / 32), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
     else if (ncol > 8 && (int64_t)gx * ((ncol + 15) / 16) >= want)
@@ -494,8 +521,8 @@ int apply_h_batch(rsdft_plan *P, int slot, int nb, const double2 *X, int64_t ldx
     const SphereTables tabs = sphere_tables(P);
     double2 *pp = P->pp[slot].p, *pq = P->pq[slot].p;
     if (nl) {   // projections read the INPUT orbitals
-        if (P->maxproj <= 8) launch_project_mt<1>(tabs, X, ldx, nb, P->dV, pp, st);
-        else launch_project_mt<2>(tabs, X, ldx, nb, P->dV, pp, st);
+        if (P->maxproj <= 8) launch_project_mt<1>(tabs, X, ldx, nb, P->dV, pp, P->num_sms, st);
+        else launch_project_mt<2>(tabs, X, ldx, nb, P->dV, pp, P->num_sms, st);
         combine_kernel<<<dim3(P->natom, (nb + NL_CCOLS - 1) / NL_CCOLS), 128, 0, st>>>(tabs, pp, nb, pq);
         P->last_launches += 2;
     }
@@ -572,7 +599,10 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
         }
         const int rc = apply_h_batch(P, slot, nb, X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx,
                                      ns > 1 ? P->s_batch[slot] : st);
-        if (rc != RSDFT_OK) return rc;
+        if (rc != RSDFT_OK) {
+            if (ns > 1) (void)join();            // keep the caller's stream ordered after whatever was queued
+            return rc;
+        }
     }
     if (ns > 1) RS_CUDA(join());
     return RSDFT_OK;
@@ -611,11 +641,8 @@ int gram_launch(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const doubl
     a.Y = Y; a.HY = HY; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = ntiles; a.kslabs = ks;
     a.nchunks = nchunks; a.tiles = dtiles; a.work = P->gram_work.p;
     auto kern = gram_dmma_kernel<2, 4, 6, 3, 16, 3>;
-    static thread_local bool attr_set = false;
-    if (!attr_set) {
-        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
-        attr_set = true;
-    }
+    // the attribute is per device/context: set it on every launch (cheap), never cache it per thread
+    RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
     kern<<<ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);
     GramReduceArgs r;
     r.work = P->gram_work.p; r.tiles = dtiles; r.H = H; r.S = S; r.n = n; r.lds = lds; r.kslabs = ks; r.ntiles = ntiles;
@@ -648,7 +675,7 @@ int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2
         if (S)
             for (int i = 0; i < tm; ++i)
                 for (int j = i; j < tm; ++j) tiles.push_back({(int16_t)i, (int16_t)j, 1, 0});
-        RS_CUDA(P->gram_tiles.upload(tiles));
+        RS_CUDA(P->gram_tiles.upload_async(tiles, st));
         P->gram_ntiles = (int)tiles.size();
         P->gram_tiles_n = key;
     }
@@ -658,7 +685,7 @@ int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2
 
 // tile list ordered by column panel (panel t = tile column t): panel t holds every [S|H] tile that
 // becomes computable when columns [0, 96(t+1)) are on the device: H(i<=t, t), H(t, j<t), S(i<=t, t).
-int gram_panel_lists(rsdft_plan *P, int n)
+int gram_panel_lists(rsdft_plan *P, int n, cudaStream_t st)
 {
     const int key = 2 * n + P->gram_h_upper;
     if (P->gram_panel_n == key) return RSDFT_OK;
@@ -672,7 +699,7 @@ int gram_panel_lists(rsdft_plan *P, int n)
         for (int i = 0; i <= t; ++i) tiles.push_back({(int16_t)i, (int16_t)t, 1, 0});
         P->gram_panel_off.push_back((int)tiles.size());
     }
-    RS_CUDA(P->gram_panel_tiles.upload(tiles));
+    RS_CUDA(P->gram_panel_tiles.upload_async(tiles, st));
     P->gram_panel_n = key;
     return RSDFT_OK;
 }
@@ -693,6 +720,8 @@ bool overlaps(const void *a, size_t na, const void *b, size_t nb)
     const char *pa = (const char *)a, *pb = (const char *)b;
     return pa < pb + nb && pb < pa + na;
 }
+
+#include "eig_driver.cuh"
 
 }  // namespace
 
@@ -747,6 +776,12 @@ int rsdft_plan_create(const rsdft_grid_t *grid, const rsdft_box_t *box, const rs
     } catch (const std::bad_alloc &) {
         rc = fail(RSDFT_ALLOC, "rsdft_plan_create: host allocation failed");
     }
+    if (rc == RSDFT_OK) {
+        // the table uploads above ran on the legacy stream: finish them before the plan can be used
+        // from a non-blocking stream
+        const cudaError_t se = cudaDeviceSynchronize();
+        if (se != cudaSuccess) rc = fail(RSDFT_CUDA, std::string("rsdft_plan_create: ") + cudaGetErrorString(se));
+    }
     if (rc != RSDFT_OK) { delete P; return rc; }
     *out = P;
     return RSDFT_OK;
@@ -763,9 +798,14 @@ int rsdft_plan_destroy(rsdft_plan_t *plan)
 int rsdft_plan_set_vloc(rsdft_plan_t *plan, const double *vloc_dev, void *stream)
 {
     if (!plan) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_vloc: null plan");
+    if (int rc = check_device(plan, "rsdft_plan_set_vloc")) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     if (vloc_dev) RS_CUDA(cudaMemcpyAsync(plan->vloc.p, vloc_dev, plan->vloc.bytes(), cudaMemcpyDeviceToDevice, st));
     else RS_CUDA(cudaMemsetAsync(plan->vloc.p, 0, plan->vloc.bytes(), st));
+    // rsdft_block_step_host runs on plan-owned streams: it orders itself after this copy through the event
+    if (!plan->ev_vloc) RS_CUDA(cudaEventCreateWithFlags(&plan->ev_vloc, cudaEventDisableTiming));
+    RS_CUDA(cudaEventRecord(plan->ev_vloc, st));
+    plan->vloc_pending = true;
     return RSDFT_OK;
 }
 
@@ -883,6 +923,11 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     RS_CUDA(P->hostHS.ensure((size_t)2 * n * n));
     if (!P->s_copy) RS_CUDA(cudaStreamCreateWithFlags(&P->s_copy, cudaStreamNonBlocking));
     if (!P->s_comp) RS_CUDA(cudaStreamCreateWithFlags(&P->s_comp, cudaStreamNonBlocking));
+    // a V_loc set on some caller stream must have landed before the plan-owned streams read it
+    if (P->vloc_pending) {
+        RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev_vloc, 0));
+        P->vloc_pending = false;
+    }
     // Column panels of one Gram tile width (96 columns): the H2D copy of panel k+1 overlaps apply_h and
     // the Gram tiles of panel k.  After panel t has been through H, every [S|H] tile that involves only
     // columns < 96(t+1) and touches panel t is contracted, so the Gram (the long part of the step) runs
@@ -894,7 +939,7 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
         RS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
         P->ev.push_back(e);
     }
-    int rc = gram_panel_lists(P, n);
+    int rc = gram_panel_lists(P, n, P->s_comp);
     if (rc != RSDFT_OK) return rc;
     size_t need = 0;
     for (int k = 0; k < nchunk; ++k) need = std::max(need, gram_work_need(P, P->gram_panel_off[k + 1] - P->gram_panel_off[k]));
@@ -902,38 +947,159 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     double2 *Hd = P->hostHS.p, *Sd = P->hostHS.p + (size_t)n * n;
     P->last_launches = 0;
     int64_t launches = 0;
-    for (int k = 0; k < nchunk; ++k) {
-        const int c0 = k * chunk, nc = std::min(chunk, n - c0);
-        RS_CUDA(cudaMemcpy2DAsync(P->hostY.p + (int64_t)c0 * ng, (size_t)ng * 16,
-                                  (const char *)Y_host + (size_t)c0 * ldy * 16, (size_t)ldy * 16, (size_t)ng * 16, nc,
-                                  cudaMemcpyHostToDevice, P->s_copy));
-        RS_CUDA(cudaEventRecord(P->ev[2 * k], P->s_copy));
-        RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev[2 * k], 0));
-        rc = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, P->s_comp);
-        if (rc != RSDFT_OK) return rc;
-        RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], P->s_comp));
-        launches += P->last_launches;
-        P->last_launches = 0;
-        rc = gram_launch(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->gram_panel_tiles.p + P->gram_panel_off[k],
-                         P->gram_panel_off[k + 1] - P->gram_panel_off[k], P->s_comp);
-        if (rc != RSDFT_OK) return rc;
-        launches += P->last_launches;
-        P->last_launches = 0;
-    }
-    P->last_launches = launches;
-    RS_CUDA(cudaMemcpy2DAsync(H_sub_host, (size_t)lds * 16, Hd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
-    RS_CUDA(cudaMemcpy2DAsync(S_sub_host, (size_t)lds * 16, Sd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
-    if (HY_host) {   // HY goes back on the copy stream, behind the uploads, while the Gram runs
+    // everything below is queued on the two plan-owned streams; on ANY error both are drained before the
+    // call returns, so no copy or kernel of a failed call is still touching the caller's host buffers
+    auto body = [&]() -> int {
         for (int k = 0; k < nchunk; ++k) {
             const int c0 = k * chunk, nc = std::min(chunk, n - c0);
-            RS_CUDA(cudaStreamWaitEvent(P->s_copy, P->ev[2 * k + 1], 0));
-            RS_CUDA(cudaMemcpy2DAsync((char *)HY_host + (size_t)c0 * ldhy * 16, (size_t)ldhy * 16,
-                                      P->hostHY.p + (int64_t)c0 * ng, (size_t)ng * 16, (size_t)ng * 16, nc,
-                                      cudaMemcpyDeviceToHost, P->s_copy));
+            RS_CUDA(cudaMemcpy2DAsync(P->hostY.p + (int64_t)c0 * ng, (size_t)ng * 16,
+                                      (const char *)Y_host + (size_t)c0 * ldy * 16, (size_t)ldy * 16, (size_t)ng * 16, nc,
+                                      cudaMemcpyHostToDevice, P->s_copy));
+            RS_CUDA(cudaEventRecord(P->ev[2 * k], P->s_copy));
+            RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev[2 * k], 0));
+            int r = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, P->s_comp);
+            if (r != RSDFT_OK) return r;
+            RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], P->s_comp));
+            launches += P->last_launches;
+            P->last_launches = 0;
+            r = gram_launch(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->gram_panel_tiles.p + P->gram_panel_off[k],
+                            P->gram_panel_off[k + 1] - P->gram_panel_off[k], P->s_comp);
+            if (r != RSDFT_OK) return r;
+            launches += P->last_launches;
+            P->last_launches = 0;
         }
+        P->last_launches = launches;
+        RS_CUDA(cudaMemcpy2DAsync(H_sub_host, (size_t)lds * 16, Hd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
+        RS_CUDA(cudaMemcpy2DAsync(S_sub_host, (size_t)lds * 16, Sd, (size_t)n * 16, (size_t)n * 16, n, cudaMemcpyDeviceToHost, P->s_comp));
+        if (HY_host) {   // HY goes back on the copy stream, behind the uploads, while the Gram runs
+            for (int k = 0; k < nchunk; ++k) {
+                const int c0 = k * chunk, nc = std::min(chunk, n - c0);
+                RS_CUDA(cudaStreamWaitEvent(P->s_copy, P->ev[2 * k + 1], 0));
+                RS_CUDA(cudaMemcpy2DAsync((char *)HY_host + (size_t)c0 * ldhy * 16, (size_t)ldhy * 16,
+                                          P->hostHY.p + (int64_t)c0 * ng, (size_t)ng * 16, (size_t)ng * 16, nc,
+                                          cudaMemcpyDeviceToHost, P->s_copy));
+            }
+        }
+        return RSDFT_OK;
+    };
+    rc = body();
+    const cudaError_t e1 = cudaStreamSynchronize(P->s_comp), e2 = cudaStreamSynchronize(P->s_copy);
+    if (rc != RSDFT_OK) return rc;
+    RS_CUDA(e1);
+    RS_CUDA(e2);
+    return RSDFT_OK;
+}
+
+int rsdft_subspace_rotate2(rsdft_plan_t *plan, int32_t n, int32_t m, const void *Y, int64_t ldy, const void *HY, int64_t ldhy,
+                           const void *Cmat, int32_t ldc, const double *lambda, void *Xout, int64_t ldx, void *HXout, int64_t ldhx,
+                           void *R, int64_t ldr, void *stream)
+{
+    if (!plan || !Y || !HY || !Cmat) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: null argument");
+    if (!Xout && !HXout && !R) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: all outputs null");
+    if (R && !lambda) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: R requested without lambda");
+    if (n <= 0 || m <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: n, m must be > 0");
+    const int64_t ng = plan->ng;
+    if (ldy < ng || ldhy < ng || (Xout && ldx < ng) || (HXout && ldhx < ng) || (R && ldr < ng))
+        return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: ld < Ng");
+    if (ldc < n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: ldc < n");
+    if (((uintptr_t)Y | (uintptr_t)HY | (uintptr_t)Cmat | (uintptr_t)Xout | (uintptr_t)HXout | (uintptr_t)R) & 15)
+        return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: pointers must be 16-byte aligned");
+    const size_t by = ((size_t)(n - 1) * ldy + ng) * 16, bh = ((size_t)(n - 1) * ldhy + ng) * 16;
+    const void *outs[3] = {Xout, HXout, R};
+    const int64_t lds3[3] = {ldx, ldhx, ldr};
+    for (int i = 0; i < 3; ++i) {
+        if (!outs[i]) continue;
+        const size_t bo = ((size_t)(m - 1) * lds3[i] + ng) * 16;
+        if (overlaps(Y, by, outs[i], bo) || overlaps(HY, bh, outs[i], bo))
+            return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: an output overlaps Y or HY");
+        for (int j = i + 1; j < 3; ++j)
+            if (outs[j] && overlaps(outs[i], bo, outs[j], ((size_t)(m - 1) * lds3[j] + ng) * 16))
+                return fail(RSDFT_INVALID_ARG, "rsdft_subspace_rotate2: outputs overlap each other");
     }
-    RS_CUDA(cudaStreamSynchronize(P->s_comp));
-    RS_CUDA(cudaStreamSynchronize(P->s_copy));
+    if (int rc = check_device(plan, "rsdft_subspace_rotate2")) return rc;
+    Rotate2Args a;
+    a.Y = (const double2 *)Y; a.HY = (const double2 *)HY; a.C = (const double2 *)Cmat; a.lambda = lambda;
+    a.X = (double2 *)Xout; a.HX = (double2 *)HXout; a.R = (double2 *)R;
+    a.ldy = ldy; a.ldhy = ldhy; a.ldx = ldx; a.ldhx = ldhx; a.ldr = ldr; a.ng = ng; a.n = n; a.m = m; a.ldc = ldc;
+    // 96 x 48 or 96 x 64 output tile (rows x columns), whichever pads m less (m = 480 -> 48, m = 512 -> 64)
+    using R48 = Rotate2Cfg<4, 2, 3, 3, 16, 3>;
+    using R64 = Rotate2Cfg<4, 2, 3, 4, 16, 3>;
+    const bool wide = ((m + 63) / 64) * 64 <= ((m + 47) / 48) * 48;
+    const int tm = R48::TM, tn = wide ? R64::TN : R48::TN;
+    a.jtiles = (m + tn - 1) / tn;
+    const int64_t units = ((ng + tm - 1) / tm) * a.jtiles;
+    if (units > 0x7fffffffll) return fail(RSDFT_UNSUPPORTED, "rsdft_subspace_rotate2: too many tiles for one launch");
+    if (wide) {
+        auto kern = rotate2_dmma_kernel<4, 2, 3, 4, 16, 3>;
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R64::SMEM));
+        kern<<<(unsigned)units, R64::THREADS, R64::SMEM, (cudaStream_t)stream>>>(a);
+    } else {
+        auto kern = rotate2_dmma_kernel<4, 2, 3, 3, 16, 3>;
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R48::SMEM));
+        kern<<<(unsigned)units, R48::THREADS, R48::SMEM, (cudaStream_t)stream>>>(a);
+    }
+    plan->last_launches = 1;
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
+}
+
+int rsdft_subspace_eig(rsdft_plan_t *plan, int32_t n, const void *H_sub, const void *S_sub, int32_t lds, int32_t m,
+                       double *lambda, void *Cmat, int32_t ldc, void *stream)
+{
+    if (!plan || !H_sub || !S_sub || !lambda || !Cmat) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig: null argument");
+    if (n <= 0 || n > 16384) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig: n out of range (1..16384)");
+    if (m <= 0 || m > n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig: m must be in 1..n");
+    if (lds < n || ldc < n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig: leading dimension < n");
+    if (((uintptr_t)H_sub | (uintptr_t)S_sub | (uintptr_t)Cmat) & 15 || ((uintptr_t)lambda & 7))
+        return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig: misaligned pointer");
+    if (int rc = check_device(plan, "rsdft_subspace_eig")) return rc;
+    plan->last_launches = 0;
+    const int rc = eig_impl(plan, n, (const double2 *)H_sub, (const double2 *)S_sub, lds, m, lambda, (double2 *)Cmat, ldc,
+                            (cudaStream_t)stream);
+    if (rc != RSDFT_OK) cudaStreamSynchronize((cudaStream_t)stream);      // nothing of a failed call stays in flight
+    return rc;
+}
+
+int rsdft_subspace_eig_get(rsdft_plan_t *plan, int32_t what, void *out, int32_t ld, void *stream)
+{
+    if (!plan || !out) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig_get: null argument");
+    if (plan->eg_n <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig_get: no successful rsdft_subspace_eig on this plan yet");
+    if (what != 0 && what != 1) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig_get: what must be 0 (L) or 1 (K)");
+    if (ld < plan->eg_n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig_get: ld < n");
+    if (int rc = check_device(plan, "rsdft_subspace_eig_get")) return rc;
+    const int n = plan->eg_n;
+    mat_copy_kernel<<<296, 256, 0, (cudaStream_t)stream>>>(what == 0 ? plan->eg_L.p : plan->eg_Z.p, n, (double2 *)out, ld, n, n, what == 0 ? 1 : 0);
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
+}
+
+int rsdft_plan_set_eig_mode(rsdft_plan_t *plan, int32_t reduction, int32_t inner_sweeps)
+{
+    if (!plan || (reduction != 0 && reduction != 1) || inner_sweeps < 0 || inner_sweeps > 16)
+        return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_eig_mode: reduction must be 0 or 1, inner_sweeps in 0..16");
+    plan->eig_mode = reduction;
+    plan->eig_inner = inner_sweeps == 0 ? 1 : inner_sweeps;
+    return RSDFT_OK;
+}
+
+int rsdft_subspace_eig_stats(const rsdft_plan_t *plan, double *out8)
+{
+    if (!plan || !out8) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_eig_stats: null argument");
+    for (int i = 0; i < 8; ++i) out8[i] = plan->eig_stats[i];
+    return RSDFT_OK;
+}
+
+int rsdft_plan_release_workspace(rsdft_plan_t *plan)
+{
+    if (!plan) return fail(RSDFT_INVALID_ARG, "rsdft_plan_release_workspace: null plan");
+    if (int rc = check_device(plan, "rsdft_plan_release_workspace")) return rc;
+    RS_CUDA(cudaDeviceSynchronize());
+    plan->hostY.release(); plan->hostHY.release(); plan->hostHS.release();
+    plan->gram_work.release();
+    for (int i = 0; i < rsdft_plan::MAX_STREAMS; ++i) { plan->pp[i].release(); plan->pq[i].release(); }
+    plan->eg_L.release(); plan->eg_B.release(); plan->eg_Z.release(); plan->eg_Dinv.release(); plan->eg_Kp.release();
+    plan->eg_Tp.release(); plan->eg_V0.release(); plan->eg_V1.release(); plan->eg_J.release(); plan->eg_Zs.release();
+    plan->eg_n = 0;
     return RSDFT_OK;
 }
 

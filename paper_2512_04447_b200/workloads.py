@@ -87,16 +87,19 @@ def gaussian_vloc(n, L, pos, depth, width):
 
 
 def sphere_margin(system):
-    """min over atoms and grid points of | |d|^2 - rc^2 | (input-validity check only:
-    the oracle and the plan must agree on sphere membership point for point)."""
+    """min over atoms and grid points of | |d|^2 - rc^2 |: an input-validity check (the oracle and the plan must
+    agree on sphere membership point for point).  Only the grid points within rc + 2h of an atom along each axis
+    can come near its sphere boundary, so each atom scans its own bounding box."""
     n, L = system["n"], system["len"]
     best = np.inf
     for a, R in enumerate(system["pos"]):
         rc = system["species"][system["species_of"][a]]["rc"]
         d2 = 0.0
         for ax in range(3):
-            r = np.arange(n[ax]) * (L[ax] / n[ax])
+            h = L[ax] / n[ax]
+            r = np.arange(n[ax]) * h
             d = _min_image(r - R[ax], L[ax])
+            d = d[np.abs(d) <= rc + 2.0 * h]
             shape = [1, 1, 1]; shape[ax] = -1
             d2 = d2 + (d * d).reshape(shape)
         best = min(best, float(np.min(np.abs(d2 - rc * rc))))
@@ -117,7 +120,7 @@ def make_system(cfg_id, with_vloc=True, check_margin=None):
     if with_vloc:
         system["vloc"] = gaussian_vloc(n, L, pos, cfg["depth"], cfg["width"])
     if check_margin is None:
-        check_margin = cfg["n"] <= 48
+        check_margin = True
     if check_margin:
         assert sphere_margin(system) > 1e-9, "grid point on a sphere boundary; change the seed"
     return system
@@ -141,6 +144,35 @@ def small_system(n=(12, 10, 8), L=(7.0, 6.0, 5.0), natom=3, seed=7, nproj=9, rc=
                   species_of=np.zeros(natom, np.int32), species=[sp], m=4, seed=seed,
                   vloc=rng.standard_normal(int(np.prod(n))))
     return system
+
+
+def subspace_pencil(n, seed, degenerate=False):
+    """Seeded synthetic (H_sub, S_sub) pencil of size n for the eigen-solve (NEXT-1), shaped like the Gram matrices
+    of a random orbital block: S = G^H G (Hermitian positive definite, well conditioned), H = G^H diag(d) G with
+    d in (-1, 3) (the Ritz values then lie in (-1, 3)).  degenerate=True builds H = B^H diag(w) B, S = B^H B with
+    repeated levels in w (shells of 6, 12, 8 like the free-electron spectrum), returning w as a third value.
+    An INPUT generator: it draws random matrices and multiplies them; it holds no step of the eigen-solve."""
+    rng = np.random.default_rng(1000003 * int(seed) + int(n))
+    cn = lambda *shape: (rng.standard_normal(shape) + 1j * rng.standard_normal(shape)) * np.sqrt(0.5)
+    if degenerate:
+        B = cn(n, n) + 2.0 * np.sqrt(n) * np.eye(n)
+        base = np.sort(rng.uniform(-1.0, 3.0, n))
+        w = base.copy()
+        i = 1
+        for deg in (6, 12, 8, 6, 24):
+            if i + deg <= n:
+                w[i:i + deg] = base[i]
+            i += deg + 3
+        w = np.sort(w)
+        H = B.conj().T @ (w[:, None] * B)
+        S = B.conj().T @ B
+        return 0.5 * (H + H.conj().T), 0.5 * (S + S.conj().T), w
+    k = 4 * n
+    G = cn(k, n)
+    d = rng.uniform(-1.0, 3.0, k)
+    S = G.conj().T @ G
+    H = G.conj().T @ (d[:, None] * G)
+    return 0.5 * (H + H.conj().T), 0.5 * (S + S.conj().T)
 
 
 def orbital_block(ng, cols, seed, stream, device="cpu", ld=None, out=None):
