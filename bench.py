@@ -48,6 +48,7 @@ def parse():
     ap.add_argument("--batch", type=int, default=0, help="apply_h column batch width (0 = library default)")
     ap.add_argument("--streams", type=int, default=0, help="apply_h internal streams (0 = library default)")
     ap.add_argument("--ncol-per-call", type=int, default=0, help="columns per rsdft_apply_h call (config 4 sweep)")
+    ap.add_argument("--pipeline", type=int, default=-1, help="apply_h FFT path: 0 three kernels per batch, 1 persistent pipeline kernel (-1 = library default)")
     return ap.parse_args()
 
 
@@ -251,6 +252,8 @@ def run_ours(args):
         rsdft.rsdft_plan_set_batch(plan, args.batch)
     if args.streams:
         rsdft.rsdft_plan_set_streams(plan, args.streams)
+    if args.pipeline >= 0:
+        rsdft.rsdft_plan_set_pipeline(plan, args.pipeline)
     peaks = probe_peaks() if rank == 0 else None
 
     # Y = [X, W, P] resident in HBM (seeded per column; every rank draws the same block)

@@ -36,7 +36,7 @@ extern "C" {
 typedef enum {
     RSDFT_OK = 0,
     RSDFT_INVALID_ARG = -1, /* null pointer, ncol <= 0, ld < Ng, X aliases HX, |m| > l, l > 2, ... */
-    RSDFT_UNSUPPORTED = -2, /* grid length outside {16,...,128 step 16, 160, 192, 256}; box <= 0; 2*rc >= min L */
+    RSDFT_UNSUPPORTED = -2, /* grid length not 16*M (M = 1..8, 10, 12, 16) nor 12*M (M = 1, 2, 3, 5, 6, 7, 10, 12); box <= 0; 2*rc >= min L */
     RSDFT_ALLOC = -3,       /* host or device allocation failed */
     RSDFT_CUDA = -4,        /* CUDA runtime error; message carries cudaGetErrorString */
     RSDFT_NOT_POSITIVE_DEFINITE = -5, /* rsdft_subspace_eig: the Cholesky factorisation of S_sub met a pivot <= 0 */
@@ -203,6 +203,13 @@ int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols);
  * Batches are independent, so results do not depend on this setting (bitwise).
  * Errors: INVALID_ARG. */
 int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams);
+
+/* apply_h FFT path.  0: three FFT kernels per column batch (every kernel makes one HBM round trip of the batch).
+ * 1: ONE persistent kernel per call that walks (column, phase, tile) work items in dependency order so that the
+ * k-space of about three columns stays in L2 between the forward, x and inverse programs; available for cubic grids
+ * of length 48, 60, 64, 80, 96, 112, 128 (other grids silently use path 0).  Results are bitwise identical.
+ * Errors: INVALID_ARG. */
+int rsdft_plan_set_pipeline(rsdft_plan_t *plan, int32_t mode);
 
 /* Gram mode.  0 (default): H_sub = Y^H (HY) is contracted in full, as the definition reads (and as the
  * paper's ZGEMM does), so it is Hermitian only to round-off.  1: only the upper 96-column

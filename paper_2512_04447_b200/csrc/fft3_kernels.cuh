@@ -1,27 +1,34 @@
-// Batched 3-D complex128 FFT Laplacian + local potential of rsdft_apply_h in THREE kernels
-// (PAPER.md:19 task (1) "FFT used to apply the Laplacian", PAPER.md:103-109 batched transforms;
-// SURVEY 8(a) a1-a4).  One HBM/L2 round trip per kernel: 3 x (16 + 16) B per orbital*point, plus
-// the 16 B re-read of psi for v(r) psi(r).
+// Batched 3-D complex128 FFT Laplacian + local potential of rsdft_apply_h (PAPER.md:19 task (1) "FFT used to apply the
+// Laplacian", PAPER.md:103-109 batched transforms).
 //
-// Every axis length is N = 16*M (M = 1..8, 10, 12, 16).  Two 1-D decompositions are used (W_N = e^{-2 pi i/N}):
-//   "M-first"  (z and x axes):  n = n1*16 + n2,  k = k1 + M*k2,
-//        X[k] = sum_n2 W_16^{n2 k2} [ W_N^{n2 k1} sum_n1 W_M^{n1 k1} x[n1*16 + n2] ]
-//        stage A = radix-M over n1 (+ twiddle), stage B = radix-16 over n2; in place, so k-space
-//        position p = k1*16 + k2 holds frequency k1 + M*k2.
-//   "16-first" (y axis, split ACROSS kernels):  n = n1*M + n2,  k = k1 + 16*k2,
-//        X[k] = sum_n2 W_M^{n2 k2} [ W_N^{n2 k1} sum_n1 W_16^{n1 k1} x[n1*M + n2] ]
-//        stage A = radix-16 over the 16 rows {n1*M + n2} (stride M)   -> kernels zy / yz
-//        stage B = radix-M  over the M CONTIGUOUS rows {k1*M + n2}    -> kernel x
-//        in place, so row r = k1*M + k2 holds frequency k1 + 16*k2.
+// Every axis length is N = R2*M with R2 = 16 (M = 1..8, 10, 12, 16) or, when 16 does not divide N, R2 = 12
+// (M = 1, 2, 3, 5, 6, 7, 10, 12: 12, 24, 36, 60 -- the paper's own 60^3 grid, PAPER.md:77 --, 72, 84, 120, 144).
+// Two 1-D decompositions are used (W_N = e^{-2 pi i/N}):
+//   "M-first"  (z and x axes):  n = n1*R2 + n2,  k = k1 + M*k2,
+//        X[k] = sum_n2 W_R2^{n2 k2} [ W_N^{n2 k1} sum_n1 W_M^{n1 k1} x[n1*R2 + n2] ]
+//        stage A = radix-M over n1 (+ twiddle), stage B = radix-R2 over n2; in place, so k-space
+//        position p = k1*R2 + k2 holds frequency k1 + M*k2.
+//   "R2-first" (y axis, split ACROSS kernels):  n = n1*M + n2,  k = k1 + R2*k2,
+//        X[k] = sum_n2 W_M^{n2 k2} [ W_N^{n2 k1} sum_n1 W_R2^{n1 k1} x[n1*M + n2] ]
+//        stage A = radix-R2 over the R2 rows {n1*M + n2} (stride M)   -> tiles zy / yz
+//        stage B = radix-M  over the M CONTIGUOUS rows {k1*M + n2}    -> tile x
+//        in place, so row r = k1*M + k2 holds frequency k1 + R2*k2.
 // k-space therefore lives in a permuted order; the kinetic table is permuted to match on the host.
 //
-//   fft3_fwd_zy_kernel  tile = (column, x, n2y): 16 rows x Nz.   z forward (A, B), y forward stage A.
-//   fft3_x_kernel       tile = (column, k1y, z-chunk): Nx x M_y rows x TZ.  y forward stage B,
-//                       x forward (A, B), multiply by t(k)/Ng, x inverse (B', A'), y inverse stage B'.
-//   fft3_inv_yz_kernel  tile = (column, x, n2y).  y inverse stage A', z inverse (B', A'),
-//                       HX = T psi + v(r) psi(r).
+// Three tile programs (device functions; a "group" is the set of threads working on one tile, synchronised by a
+// named barrier, so that two groups of one CTA can run two tiles side by side):
+//   fft3_fwd_tile   tile = (column, x, n2y): R2y rows x Nz.   z forward (A, B), y forward stage A.
+//   fft3_x_tile     tile = (column, k1y, z-chunk): Nx x M_y rows x TZ.  y forward stage B, x forward (A, B),
+//                   multiply by t(k)/Ng, x inverse (B', A'), y inverse stage B'.
+//   fft3_inv_tile   tile = (column, x, n2y).  y inverse stage A', z inverse (B', A'), HX = T psi + v(r) psi(r).
+// and two ways to run them:
+//   * three kernels per column batch (fft3_fwd_zy_kernel, fft3_x_kernel, fft3_inv_yz_kernel): every kernel makes one
+//     HBM round trip of the batch;
+//   * ONE persistent kernel (fft3_pipeline_kernel) that walks (column, phase, tile) work items from an in-order queue
+//     with per-column completion counters, keeping about three columns of k-space in flight so that the hand-over
+//     fwd -> x -> inv goes through L2 instead of HBM (north_star "one HBM round trip per direction").
 // The inverse transform is the forward codelet run on (im, re)-swapped data.
-// All global accesses are >= 128 B contiguous segments of 16 B elements.
+// All global accesses are >= 64 B contiguous segments of 16 B elements.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -31,118 +38,225 @@
 namespace rsdft {
 
 struct Fft3Args {
-    const double2 *X;       // input orbitals (zy source; yz: psi for the V_loc term)
+    const double2 *X;       // input orbitals (fwd source; inv: psi for the V_loc term)
     double2 *W;             // k-space scratch, same layout as a column block (may be HX itself)
-    double2 *HX;            // output of the yz kernel
+    double2 *HX;            // output of the inv tiles
     int64_t ldx, ldw, ldhx; // column strides (elements)
     int32_t ncol, nx, ny, nz;
-    int32_t my;             // ny / 16
+    int32_t my;             // ny / R2y
+    int32_t r2y;            // 16 or 12
     const double2 *twx, *twy, *twz;   // w_N^m = (cos, -sin)(2 pi m / N), m in [0, N)
     const double *kin_x;    // [nx]     t_x(kx)/Ng, natural frequency index
     const double *kin_yz;   // [ny*nz]  (t_y(ky(r)) + t_z(kz(p)))/Ng at r*nz + p (permuted positions)
     const double *vloc;     // [Ng]
 };
 
-__device__ __forceinline__ double2 ld_nc(const double2 *p) { return __ldg(p); }
-
-// ---------------------------------------------------------------------------------------------
-// shared-memory geometry of the 16-row tiles of the zy / yz kernels
-template <int NZ>
-struct ZyCfg {
-    static constexpr int MZ = NZ / 16;
-    static constexpr int RP = MZ * 17;                 // smem row pitch: 17 slots per 16-point group
-    static constexpr int TILE = 16 * RP;               // double2 elements per tile buffer
-    static constexpr size_t SMEM_FWD = (size_t)TILE * sizeof(double2);
-    static constexpr size_t SMEM_INV = (size_t)(2 * TILE + 16 * NZ) * sizeof(double2);
+constexpr bool radix16_ok(int N) { return N % 16 == 0 && (N / 16 <= 8 || N / 16 == 10 || N / 16 == 12 || N / 16 == 16); }
+template <int N> struct Axis {
+    static constexpr int R2 = radix16_ok(N) ? 16 : 12;
+    static constexpr int M = N / R2;
+    static_assert(N % R2 == 0, "axis length must be a multiple of 16 or of 12");
 };
 
+__device__ __forceinline__ double2 ld_nc(const double2 *p) { return __ldg(p); }
+// k-space is written by other SMs inside one launch of the pipeline kernel: read it through L2 only
+__device__ __forceinline__ double2 ld_cg(const double2 *p) { return __ldcg(p); }
+
+// barrier `id` over `nt` threads (id 0 with the whole CTA = __syncthreads)
+__device__ __forceinline__ void group_sync(int id, int nt) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nt) : "memory"); }
+
+// ---------------------------------------------------------------------------------------------
+// shared-memory geometry of the R2y-row tiles of the fwd / inv programs
+template <int NZ, int R2Y>
+struct ZyCfg {
+    static constexpr int R2Z = Axis<NZ>::R2, MZ = Axis<NZ>::M;
+    static constexpr int G = R2Z + 1;                  // slots per R2Z-point group (odd: conflict-free columns)
+    static constexpr int RP = MZ * G;                  // smem row pitch
+    static constexpr int TILE = R2Y * RP;              // double2 elements per tile buffer
+    static constexpr int NTWZ = (MZ > 1 ? MZ - 1 : 1) * R2Z;
+    static constexpr size_t SMEM_FWD = (size_t)TILE * sizeof(double2);
+    static constexpr size_t SMEM_INV = (size_t)(2 * TILE + R2Y * NZ) * sizeof(double2);
+};
+
+// twiddle tables of a fwd / inv tile: twz_s[(k-1)*R2Z + n2] = w_NZ^{n2 k}, twy_s[k] = w_NY^{n2y k}
+template <int NZ, int R2Y, int NT>
+__device__ __forceinline__ void fft3_zy_tables(const Fft3Args &a, int n2y, double2 *twz_s, double2 *twy_s, int tid, bool want_z)
+{
+    constexpr int R2Z = Axis<NZ>::R2, MZ = Axis<NZ>::M;
+    if (want_z)
+        for (int e = tid; e < (MZ - 1) * R2Z; e += NT) twz_s[e] = a.twz[(e % R2Z) * (e / R2Z + 1)];
+    if (tid < R2Y) twy_s[tid] = a.twy[n2y * tid];
+}
+
+// z forward + y forward stage A of one tile.  src/dst: plane base (column, x) of X / W.
+template <int NZ, int R2Y, int NT>
+__device__ __forceinline__ void fft3_fwd_tile(const double2 *__restrict__ src, double2 *__restrict__ dst, int my, int n2y, double2 *S,
+                                              const double2 *twz_s, const double2 *twy_s, int tid, int bar)
+{
+    using C = ZyCfg<NZ, R2Y>;
+    constexpr int R2Z = C::R2Z, MZ = C::MZ, G = C::G, RP = C::RP;
+    // z stage A: radix-MZ over n1, twiddle w_NZ^{n2 k1}
+#pragma unroll
+    for (int item = tid; item < R2Y * R2Z; item += NT) {
+        const int j = item / R2Z, n2 = item % R2Z;
+        const double2 *row = src + (int64_t)(j * my + n2y) * NZ + n2;
+        double re[MZ], im[MZ];
+#pragma unroll
+        for (int n1 = 0; n1 < MZ; ++n1) { const double2 v = ld_nc(row + n1 * R2Z); re[n1] = v.x; im[n1] = v.y; }
+        Dft<MZ>::run(re, im);
+#pragma unroll
+        for (int k = 1; k < MZ; ++k) { const double2 w = twz_s[(k - 1) * R2Z + n2]; tw_mul(re[k], im[k], w.x, -w.y); }
+#pragma unroll
+        for (int k = 0; k < MZ; ++k) S[j * RP + k * G + n2] = make_double2(re[k], im[k]);
+    }
+    group_sync(bar, NT);
+    // z stage B: radix-R2Z over n2, in place (position k1*R2Z + k2 <- frequency k1 + MZ*k2)
+    for (int item = tid; item < R2Y * MZ; item += NT) {
+        double2 *p = S + item * G;
+        double br[R2Z], bi[R2Z];
+#pragma unroll
+        for (int t = 0; t < R2Z; ++t) { const double2 v = p[t]; br[t] = v.x; bi[t] = v.y; }
+        Dft<R2Z>::run(br, bi);
+#pragma unroll
+        for (int t = 0; t < R2Z; ++t) p[t] = make_double2(br[t], bi[t]);
+    }
+    group_sync(bar, NT);
+    // y stage A: radix-R2Y over the R2Y rows, twiddle w_NY^{n2y k1}, store row k1*my + n2y
+    for (int p = tid; p < NZ; p += NT) {
+        const int sp = (p / R2Z) * G + (p % R2Z);
+        double br[R2Y], bi[R2Y];
+#pragma unroll
+        for (int j = 0; j < R2Y; ++j) { const double2 v = S[j * RP + sp]; br[j] = v.x; bi[j] = v.y; }
+        Dft<R2Y>::run(br, bi);
+#pragma unroll
+        for (int k = 1; k < R2Y; ++k) { const double2 w = twy_s[k]; tw_mul(br[k], bi[k], w.x, -w.y); }
+#pragma unroll
+        for (int k = 0; k < R2Y; ++k) dst[(int64_t)(k * my + n2y) * NZ + p] = make_double2(br[k], bi[k]);
+    }
+    group_sync(bar, NT);
+}
+
+// y inverse stage A' and z inverse stage B' of a tile already in shared memory (padded layout)
+template <int NZ, int R2Y, int NT>
+__device__ __forceinline__ void fft3_inv_stages_12(double2 *S, const double2 *twy_s, int tid, int bar)
+{
+    using C = ZyCfg<NZ, R2Y>;
+    constexpr int R2Z = C::R2Z, MZ = C::MZ, G = C::G, RP = C::RP;
+    // y inverse stage A': conj twiddle, radix-R2Y over k1y (swapped domain) -> row j = n1y, in place
+    for (int p = tid; p < NZ; p += NT) {
+        double2 *c = S + (p / R2Z) * G + (p % R2Z);
+        double br[R2Y], bi[R2Y];
+#pragma unroll
+        for (int k = 0; k < R2Y; ++k) { const double2 v = c[k * RP]; br[k] = v.x; bi[k] = v.y; }
+#pragma unroll
+        for (int k = 1; k < R2Y; ++k) { const double2 w = twy_s[k]; tw_mul(bi[k], br[k], w.x, -w.y); }
+        Dft<R2Y>::run(bi, br);
+#pragma unroll
+        for (int j = 0; j < R2Y; ++j) c[j * RP] = make_double2(br[j], bi[j]);
+    }
+    group_sync(bar, NT);
+    // z inverse stage B': radix-R2Z over k2z (swapped), in place
+    for (int item = tid; item < R2Y * MZ; item += NT) {
+        double2 *p = S + item * G;
+        double br[R2Z], bi[R2Z];
+#pragma unroll
+        for (int q = 0; q < R2Z; ++q) { const double2 v = p[q]; br[q] = v.x; bi[q] = v.y; }
+        Dft<R2Z>::run(bi, br);
+#pragma unroll
+        for (int q = 0; q < R2Z; ++q) p[q] = make_double2(br[q], bi[q]);
+    }
+}
+
+// z inverse stage A' + V_loc: conj twiddle, radix-MZ over k1z (swapped) -> z = n1*R2Z + n2;  HX = T psi + v psi.
+// psi comes from shared memory (Sp, dense [R2Y][NZ]) when PSI_SMEM, else straight from global memory (psi_g = plane base).
+template <int NZ, int R2Y, int NT, bool PSI_SMEM>
+__device__ __forceinline__ void fft3_inv_stage_3(const double2 *S, const double2 *twz_s, const double2 *Sp, const double2 *__restrict__ psi_g,
+                                                 const double *__restrict__ vl, double2 *__restrict__ dst, int my, int n2y, int tid)
+{
+    using C = ZyCfg<NZ, R2Y>;
+    constexpr int R2Z = C::R2Z, MZ = C::MZ, G = C::G, RP = C::RP;
+#pragma unroll
+    for (int item = tid; item < R2Y * R2Z; item += NT) {
+        const int j = item / R2Z, n2 = item % R2Z;
+        const int64_t off = (int64_t)(j * my + n2y) * NZ + n2;
+        double2 ps[MZ];
+        double vv[MZ];
+#pragma unroll
+        for (int n1 = 0; n1 < MZ; ++n1) {          // issued first: their latency hides behind the radix-MZ below
+            ps[n1] = PSI_SMEM ? Sp[j * NZ + n1 * R2Z + n2] : ld_nc(psi_g + off + n1 * R2Z);
+            vv[n1] = __ldg(vl + off + n1 * R2Z);
+        }
+        double re[MZ], im[MZ];
+#pragma unroll
+        for (int k = 0; k < MZ; ++k) { const double2 v = S[j * RP + k * G + n2]; re[k] = v.x; im[k] = v.y; }
+#pragma unroll
+        for (int k = 1; k < MZ; ++k) { const double2 w = twz_s[(k - 1) * R2Z + n2]; tw_mul(im[k], re[k], w.x, -w.y); }
+        Dft<MZ>::run(im, re);
+#pragma unroll
+        for (int n1 = 0; n1 < MZ; ++n1)
+            dst[off + n1 * R2Z] = make_double2(fma(vv[n1], ps[n1].x, re[n1]), fma(vv[n1], ps[n1].y, im[n1]));
+    }
+}
+
+// cp.async of the R2Y k-space rows {k*my + n2y} of one plane into the padded tile layout
+template <int NZ, int R2Y, int NT>
+__device__ __forceinline__ void fft3_issue_w_tile(const double2 *__restrict__ src, int my, int n2y, double2 *S, int tid)
+{
+    using C = ZyCfg<NZ, R2Y>;
+    constexpr int R2Z = C::R2Z, G = C::G, RP = C::RP;
+#pragma unroll
+    for (int e = tid; e < R2Y * NZ; e += NT) {
+        const int k = e / NZ, p = e - k * NZ;
+        cp_async16(S + k * RP + (p / R2Z) * G + (p % R2Z), src + (int64_t)(k * my + n2y) * NZ + p);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // z forward + y forward stage A.  128 threads; grid = G * my, CTA b works on n2y = b % my.
-template <int NZ, int MINB>
+template <int NZ, int R2Y, int MINB>
 __global__ void __launch_bounds__(128, MINB) fft3_fwd_zy_kernel(Fft3Args a)
 {
-    constexpr int MZ = NZ / 16;
-    constexpr int RP = MZ * 17;                 // smem row pitch: 17 slots per 16-point group
+    using C = ZyCfg<NZ, R2Y>;
     constexpr int NT = 128;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2 *S = reinterpret_cast<double2 *>(smem_raw);          // [16 * RP]
-    __shared__ double2 twz_s[(MZ > 1 ? MZ - 1 : 1) * 16];
-    __shared__ double2 twy_s[16];
+    double2 *S = reinterpret_cast<double2 *>(smem_raw);
+    __shared__ double2 twz_s[C::NTWZ];
+    __shared__ double2 twy_s[R2Y];
     const int tid = threadIdx.x;
     const int my = a.my;
     const int n2y = blockIdx.x % my;
     const int g0 = blockIdx.x / my, G = gridDim.x / my;
-    for (int e = tid; e < (MZ - 1) * 16; e += NT) twz_s[e] = a.twz[(e & 15) * ((e >> 4) + 1)];
-    if (tid < 16) twy_s[tid] = a.twy[n2y * tid];
+    fft3_zy_tables<NZ, R2Y, NT>(a, n2y, twz_s, twy_s, tid, true);
     __syncthreads();
     const int64_t nplanes = (int64_t)a.ncol * a.nx;
     for (int64_t cx = g0; cx < nplanes; cx += G) {
         const int64_t col = cx / a.nx;
         const int64_t x = cx - col * a.nx;
-        const double2 *src = a.X + col * a.ldx + x * a.ny * NZ;
-        double2 *dst = a.W + col * a.ldw + x * a.ny * NZ;
-        // z stage A: radix-MZ over n1, twiddle w_NZ^{n2 k1}
-#pragma unroll
-        for (int item = tid; item < 256; item += NT) {
-            const int j = item >> 4, n2 = item & 15;
-            const double2 *row = src + (int64_t)(j * my + n2y) * NZ + n2;
-            double re[MZ], im[MZ];
-#pragma unroll
-            for (int n1 = 0; n1 < MZ; ++n1) { const double2 v = ld_nc(row + n1 * 16); re[n1] = v.x; im[n1] = v.y; }
-            Dft<MZ>::run(re, im);
-#pragma unroll
-            for (int k = 1; k < MZ; ++k) { const double2 w = twz_s[(k - 1) * 16 + n2]; tw_mul(re[k], im[k], w.x, -w.y); }
-#pragma unroll
-            for (int k = 0; k < MZ; ++k) S[j * RP + k * 17 + n2] = make_double2(re[k], im[k]);
-        }
-        __syncthreads();
-        // z stage B: radix-16 over n2, in place (position k1*16 + k2 <- frequency k1 + MZ*k2)
-        for (int item = tid; item < 16 * MZ; item += NT) {
-            double2 *p = S + item * 17;
-            double br[16], bi[16];
-#pragma unroll
-            for (int t = 0; t < 16; ++t) { const double2 v = p[t]; br[t] = v.x; bi[t] = v.y; }
-            Dft<16>::run(br, bi);
-#pragma unroll
-            for (int t = 0; t < 16; ++t) p[t] = make_double2(br[t], bi[t]);
-        }
-        __syncthreads();
-        // y stage A: radix-16 over the 16 rows, twiddle w_NY^{n2y k1}, store row k1*my + n2y
-        for (int p = tid; p < NZ; p += NT) {
-            const int sp = (p >> 4) * 17 + (p & 15);
-            double br[16], bi[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) { const double2 v = S[j * RP + sp]; br[j] = v.x; bi[j] = v.y; }
-            Dft<16>::run(br, bi);
-#pragma unroll
-            for (int k = 1; k < 16; ++k) { const double2 w = twy_s[k]; tw_mul(br[k], bi[k], w.x, -w.y); }
-#pragma unroll
-            for (int k = 0; k < 16; ++k) dst[(int64_t)(k * my + n2y) * NZ + p] = make_double2(br[k], bi[k]);
-        }
-        __syncthreads();
+        fft3_fwd_tile<NZ, R2Y, NT>(a.X + col * a.ldx + x * a.ny * NZ, a.W + col * a.ldw + x * a.ny * NZ, my, n2y, S, twz_s, twy_s, tid, 0);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // y inverse stage A' + z inverse + V_loc.  Mirror of the kernel above; W -> HX (may be in place:
-// a tile reads and writes the same 16 rows).  CTA b owns n2y = b % my and the x planes
-// g0, g0 + G, ...; for each plane it runs over ALL columns of the batch (the 16 rows of v(r) stay
+// a tile reads and writes the same R2Y rows).  CTA b owns n2y = b % my and the x planes
+// g0, g0 + G, ...; for each plane it runs over ALL columns of the batch (the rows of v(r) stay
 // hot in L1/L2).  Per tile: the k-space rows of the NEXT tile (double buffered) and the psi rows of
 // THIS tile (consumed two phases later) arrive by cp.async.
-template <int NZ, int MINB>
+template <int NZ, int R2Y, int MINB>
 __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
 {
-    constexpr int MZ = ZyCfg<NZ>::MZ, RP = ZyCfg<NZ>::RP, TILE = ZyCfg<NZ>::TILE, NT = 128;
+    using C = ZyCfg<NZ, R2Y>;
+    constexpr int TILE = C::TILE, NT = 128;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2 *Sw0 = reinterpret_cast<double2 *>(smem_raw);
-    double2 *Sp = Sw0 + 2 * TILE;                               // psi rows, dense [16][NZ]
-    __shared__ double2 twz_s[(MZ > 1 ? MZ - 1 : 1) * 16];
-    __shared__ double2 twy_s[16];
+    double2 *Sp = Sw0 + 2 * TILE;                               // psi rows, dense [R2Y][NZ]
+    __shared__ double2 twz_s[C::NTWZ];
+    __shared__ double2 twy_s[R2Y];
     const int tid = threadIdx.x;
     const int my = a.my;
     const int n2y = blockIdx.x % my;
     const int g0 = blockIdx.x / my, G = gridDim.x / my;
-    for (int e = tid; e < (MZ - 1) * 16; e += NT) twz_s[e] = a.twz[(e & 15) * ((e >> 4) + 1)];
-    if (tid < 16) twy_s[tid] = a.twy[n2y * tid];
+    fft3_zy_tables<NZ, R2Y, NT>(a, n2y, twz_s, twy_s, tid, true);
     const int nxm = g0 < a.nx ? (a.nx - g0 + G - 1) / G : 0;      // planes of this walker
     const int64_t T = (int64_t)nxm * a.ncol;                      // tiles: plane-major, column-minor
     auto plane_off = [&](int64_t t, int64_t &col) -> int64_t {
@@ -153,20 +267,14 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
     auto issue_w = [&](int buf, int64_t t) {
         int64_t col;
         const int64_t po = plane_off(t, col);
-        const double2 *src = a.W + col * a.ldw + po;
-        double2 *S = Sw0 + buf * TILE;
-#pragma unroll
-        for (int e = tid; e < 16 * NZ; e += NT) {
-            const int k = e / NZ, p = e - k * NZ;
-            cp_async16(S + k * RP + (p >> 4) * 17 + (p & 15), src + (int64_t)(k * my + n2y) * NZ + p);
-        }
+        fft3_issue_w_tile<NZ, R2Y, NT>(a.W + col * a.ldw + po, my, n2y, Sw0 + buf * TILE, tid);
     };
     auto issue_psi = [&](int64_t t) {
         int64_t col;
         const int64_t po = plane_off(t, col);
         const double2 *src = a.X + col * a.ldx + po;
 #pragma unroll
-        for (int e = tid; e < 16 * NZ; e += NT) {
+        for (int e = tid; e < R2Y * NZ; e += NT) {
             const int j = e / NZ, p = e - j * NZ;
             cp_async16(Sp + e, src + (int64_t)(j * my + n2y) * NZ + p);
         }
@@ -184,51 +292,10 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
         int64_t col;
         const int64_t po = plane_off(t, col);
         double2 *S = Sw0 + buf * TILE;
-        const double *vl = a.vloc + po;
-        double2 *dst = a.HX + col * a.ldhx + po;
-        // y inverse stage A': conj twiddle, radix-16 over k1y (swapped domain) -> row j = n1y, in place
-        for (int p = tid; p < NZ; p += NT) {
-            double2 *c = S + (p >> 4) * 17 + (p & 15);
-            double br[16], bi[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k) { const double2 v = c[k * RP]; br[k] = v.x; bi[k] = v.y; }
-#pragma unroll
-            for (int k = 1; k < 16; ++k) { const double2 w = twy_s[k]; tw_mul(bi[k], br[k], w.x, -w.y); }
-            Dft<16>::run(bi, br);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) c[j * RP] = make_double2(br[j], bi[j]);
-        }
-        __syncthreads();
-        // z inverse stage B': radix-16 over k2z (swapped), in place
-        for (int item = tid; item < 16 * MZ; item += NT) {
-            double2 *p = S + item * 17;
-            double br[16], bi[16];
-#pragma unroll
-            for (int q = 0; q < 16; ++q) { const double2 v = p[q]; br[q] = v.x; bi[q] = v.y; }
-            Dft<16>::run(bi, br);
-#pragma unroll
-            for (int q = 0; q < 16; ++q) p[q] = make_double2(br[q], bi[q]);
-        }
+        fft3_inv_stages_12<NZ, R2Y, NT>(S, twy_s, tid, 0);
         cp_async_wait<1>();                                       // psi(t) has landed
         __syncthreads();
-        // z inverse stage A': conj twiddle, radix-MZ over k1z (swapped) -> z = n1*16 + n2; + v psi
-#pragma unroll
-        for (int item = tid; item < 256; item += NT) {
-            const int j = item >> 4, n2 = item & 15;
-            double re[MZ], im[MZ];
-#pragma unroll
-            for (int k = 0; k < MZ; ++k) { const double2 v = S[j * RP + k * 17 + n2]; re[k] = v.x; im[k] = v.y; }
-#pragma unroll
-            for (int k = 1; k < MZ; ++k) { const double2 w = twz_s[(k - 1) * 16 + n2]; tw_mul(im[k], re[k], w.x, -w.y); }
-            Dft<MZ>::run(im, re);
-            const int64_t off = (int64_t)(j * my + n2y) * NZ + n2;
-#pragma unroll
-            for (int n1 = 0; n1 < MZ; ++n1) {
-                const double2 ps = Sp[j * NZ + n1 * 16 + n2];
-                const double vv = __ldg(vl + off + n1 * 16);
-                dst[off + n1 * 16] = make_double2(fma(vv, ps.x, re[n1]), fma(vv, ps.y, im[n1]));
-            }
-        }
+        fft3_inv_stage_3<NZ, R2Y, NT, true>(S, twz_s, Sp, nullptr, a.vloc + po, a.HX + col * a.ldhx + po, my, n2y, tid);
         __syncthreads();
     }
     cp_async_wait<0>();
@@ -237,7 +304,7 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
 // ---------------------------------------------------------------------------------------------
 // y stage B, x forward, kinetic factor, x inverse, y stage B'.  In place on W.
 // Tile = (column, k1y, z-chunk): S[x][line], line = jy*TZ + z, odd pitch P = lines + 1.
-template <int MY, int NX, int TZ, int NT>
+template <int MY, int NX, int TZ, int NT, bool CG>
 __device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *base, double2 *S, int P, int tid)
 {
     // items are taken two at a time so that both items' global loads are in flight together
@@ -248,9 +315,9 @@ __device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *
         const double2 *p1 = base + (int64_t)x1 * a.ny * a.nz + z1;
         double re0[MY], im0[MY], re1[MY], im1[MY];
 #pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = p0[(int64_t)j * a.nz]; re0[j] = v.x; im0[j] = v.y; }
+        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg(p0 + (int64_t)j * a.nz) : p0[(int64_t)j * a.nz]; re0[j] = v.x; im0[j] = v.y; }
 #pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = p1[(int64_t)j * a.nz]; re1[j] = v.x; im1[j] = v.y; }
+        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg(p1 + (int64_t)j * a.nz) : p1[(int64_t)j * a.nz]; re1[j] = v.x; im1[j] = v.y; }
         Dft<MY>::run(re0, im0);
 #pragma unroll
         for (int j = 0; j < MY; ++j) S[x0 * P + j * TZ + z0] = make_double2(re0[j], im0[j]);
@@ -263,7 +330,7 @@ __device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *
         const double2 *ptr = base + (int64_t)x * a.ny * a.nz + z;
         double re[MY], im[MY];
 #pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = ptr[(int64_t)j * a.nz]; re[j] = v.x; im[j] = v.y; }
+        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg(ptr + (int64_t)j * a.nz) : ptr[(int64_t)j * a.nz]; re[j] = v.x; im[j] = v.y; }
         Dft<MY>::run(re, im);
 #pragma unroll
         for (int j = 0; j < MY; ++j) S[x * P + j * TZ + z] = make_double2(re[j], im[j]);
@@ -285,119 +352,240 @@ __device__ __forceinline__ void fft3_x_store_y(const Fft3Args &a, double2 *base,
     }
 }
 
+#define RS_SWITCH_MY(MY_, CALL_)                     \
+    switch (MY_) {                                   \
+    case 1: { constexpr int MYC = 1; CALL_; } break;   \
+    case 2: { constexpr int MYC = 2; CALL_; } break;   \
+    case 3: { constexpr int MYC = 3; CALL_; } break;   \
+    case 4: { constexpr int MYC = 4; CALL_; } break;   \
+    case 5: { constexpr int MYC = 5; CALL_; } break;   \
+    case 6: { constexpr int MYC = 6; CALL_; } break;   \
+    case 7: { constexpr int MYC = 7; CALL_; } break;   \
+    case 8: { constexpr int MYC = 8; CALL_; } break;   \
+    case 10: { constexpr int MYC = 10; CALL_; } break; \
+    case 12: { constexpr int MYC = 12; CALL_; } break; \
+    default: { constexpr int MYC = 16; CALL_; } break; \
+    }
+
+// One x tile, in place on W.  base = W + column offset + (k1y*my)*nz + zc*TZ.  twx_s[(k-1)*R2X + n2] = w_NX^{n2 k},
+// kinx_s[kx] = t_x(kx)/Ng, kin = kin_yz + (k1y*my)*nz + zc*TZ.  The whole CTA (NT threads) works on the tile.
+template <int NX, int TZ, int NT, bool CG>
+__device__ __forceinline__ void fft3_x_tile(const Fft3Args &a, double2 *base, const double *__restrict__ kin, double2 *S,
+                                            const double2 *twx_s, const double *kinx_s, int tid)
+{
+    constexpr int R2X = Axis<NX>::R2, MX = Axis<NX>::M;
+    const int my = a.my, lines = my * TZ, P = lines + 1;
+    RS_SWITCH_MY(my, (fft3_x_load_y<MYC, NX, TZ, NT, CG>(a, base, S, P, tid)))
+    __syncthreads();
+    // x stage A: radix-MX over n1 (x = n1*R2X + n2), twiddle, in place
+    for (int item = tid; item < lines * R2X; item += NT) {
+        const int n2 = item % R2X, line = item / R2X;
+        double2 *p = S + n2 * P + line;
+        double re[MX], im[MX];
+#pragma unroll
+        for (int n1 = 0; n1 < MX; ++n1) { const double2 v = p[n1 * R2X * P]; re[n1] = v.x; im[n1] = v.y; }
+        Dft<MX>::run(re, im);
+#pragma unroll
+        for (int k = 1; k < MX; ++k) { const double2 w = twx_s[(k - 1) * R2X + n2]; tw_mul(re[k], im[k], w.x, -w.y); }
+#pragma unroll
+        for (int k = 0; k < MX; ++k) p[k * R2X * P] = make_double2(re[k], im[k]);
+    }
+    __syncthreads();
+    // x stage B (radix-R2X over n2) -> frequency kx = k1 + MX*k2; kinetic factor; inverse stage B'
+    for (int item = tid; item < lines * MX; item += NT) {
+        const int line = item % lines, k1 = item / lines;
+        double2 *p = S + k1 * R2X * P + line;
+        double br[R2X], bi[R2X];
+#pragma unroll
+        for (int t = 0; t < R2X; ++t) { const double2 v = p[t * P]; br[t] = v.x; bi[t] = v.y; }
+        Dft<R2X>::run(br, bi);
+        const int jy = line / TZ, z = line - jy * TZ;
+        const double tin = __ldg(kin + (int64_t)jy * a.nz + z);
+#pragma unroll
+        for (int k2 = 0; k2 < R2X; ++k2) {
+            const double f = kinx_s[k1 + MX * k2] + tin;
+            br[k2] *= f; bi[k2] *= f;
+        }
+        Dft<R2X>::run(bi, br);                  // swapped domain from here on
+#pragma unroll
+        for (int t = 0; t < R2X; ++t) p[t * P] = make_double2(br[t], bi[t]);
+    }
+    __syncthreads();
+    // x inverse stage A': conj twiddle, radix-MX over k1 -> x = n1*R2X + n2
+    for (int item = tid; item < lines * R2X; item += NT) {
+        const int n2 = item % R2X, line = item / R2X;
+        double2 *p = S + n2 * P + line;
+        double re[MX], im[MX];
+#pragma unroll
+        for (int k = 0; k < MX; ++k) { const double2 v = p[k * R2X * P]; re[k] = v.x; im[k] = v.y; }
+#pragma unroll
+        for (int k = 1; k < MX; ++k) { const double2 w = twx_s[(k - 1) * R2X + n2]; tw_mul(im[k], re[k], w.x, -w.y); }
+        Dft<MX>::run(im, re);
+#pragma unroll
+        for (int n1 = 0; n1 < MX; ++n1) p[n1 * R2X * P] = make_double2(re[n1], im[n1]);
+    }
+    __syncthreads();
+    RS_SWITCH_MY(my, (fft3_x_store_y<MYC, NX, TZ, NT>(a, base, S, P, tid)))
+    __syncthreads();
+}
+
 // Per-length launch shape: z points per tile (TZ*16 B contiguous per row), threads, CTAs per SM.
 // (NT = 288 for 96, which fills the radix-16 phase in one round, measured 40 % slower than 256.)
-template <int NX> struct XCfg;
+template <int NX> struct XCfg { static constexpr int TZ = 4, NT = 256, MINB = 1; };
+template <> struct XCfg<12> { static constexpr int TZ = 4, NT = 32, MINB = 8; };
 template <> struct XCfg<16> { static constexpr int TZ = 8, NT = 32, MINB = 8; };
+template <> struct XCfg<24> { static constexpr int TZ = 4, NT = 64, MINB = 8; };
 template <> struct XCfg<32> { static constexpr int TZ = 8, NT = 64, MINB = 8; };
+template <> struct XCfg<36> { static constexpr int TZ = 4, NT = 96, MINB = 5; };
 template <> struct XCfg<48> { static constexpr int TZ = 8, NT = 96, MINB = 5; };
+template <> struct XCfg<60> { static constexpr int TZ = 4, NT = 128, MINB = 4; };
 template <> struct XCfg<64> { static constexpr int TZ = 8, NT = 128, MINB = 4; };
+template <> struct XCfg<72> { static constexpr int TZ = 8, NT = 224, MINB = 2; };
 template <> struct XCfg<80> { static constexpr int TZ = 8, NT = 224, MINB = 2; };
+template <> struct XCfg<84> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
 template <> struct XCfg<96> { static constexpr int TZ = 8, NT = 256, MINB = 2; };
 template <> struct XCfg<112> { static constexpr int TZ = 8, NT = 256, MINB = 2; };
+template <> struct XCfg<120> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
 template <> struct XCfg<128> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
+template <> struct XCfg<144> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
 template <> struct XCfg<160> { static constexpr int TZ = 4, NT = 256, MINB = 2; };
 template <> struct XCfg<192> { static constexpr int TZ = 4, NT = 256, MINB = 1; };
 template <> struct XCfg<256> { static constexpr int TZ = 2, NT = 256, MINB = 1; };
 
+template <int NX> struct XTables {
+    static constexpr int R2X = Axis<NX>::R2, MX = Axis<NX>::M;
+    static constexpr int NTW = (MX > 1 ? MX - 1 : 1) * R2X;
+};
+
+template <int NX, int NT>
+__device__ __forceinline__ void fft3_x_tables(const Fft3Args &a, double2 *twx_s, double *kinx_s, int tid)
+{
+    constexpr int R2X = Axis<NX>::R2, MX = Axis<NX>::M;
+    for (int e = tid; e < (MX - 1) * R2X; e += NT) twx_s[e] = a.twx[(e % R2X) * (e / R2X + 1)];
+    for (int e = tid; e < NX; e += NT) kinx_s[e] = a.kin_x[e];
+}
+
 template <int NX, int TZ, int NT, int MINB>
 __global__ void __maxnreg__(((65536 / (NT * MINB)) / 8 * 8) > 255 ? 255 : ((65536 / (NT * MINB)) / 8 * 8)) fft3_x_kernel(Fft3Args a)
 {
-    constexpr int MX = NX / 16;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2 *S = reinterpret_cast<double2 *>(smem_raw);
-    __shared__ double2 twx_s[(MX > 1 ? MX - 1 : 1) * 16];
+    __shared__ double2 twx_s[XTables<NX>::NTW];
     __shared__ double kinx_s[NX];
     const int tid = threadIdx.x;
-    const int my = a.my, lines = my * TZ, P = lines + 1;
-    for (int e = tid; e < (MX - 1) * 16; e += NT) twx_s[e] = a.twx[(e & 15) * ((e >> 4) + 1)];
-    for (int e = tid; e < NX; e += NT) kinx_s[e] = a.kin_x[e];
+    const int my = a.my;
+    fft3_x_tables<NX, NT>(a, twx_s, kinx_s, tid);
     __syncthreads();
     const int zchunks = a.nz / TZ;
-    const int64_t per_col = (int64_t)16 * zchunks;
+    const int64_t per_col = (int64_t)a.r2y * zchunks;
     const int64_t ntiles = per_col * a.ncol;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int64_t colf = tile / per_col;
         const int rem = (int)(tile - colf * per_col);
         const int64_t col = a.ncol - 1 - colf;     // zig-zag: the forward kernel ended on the last column, start there (L2)
         const int k1y = rem / zchunks, zc = rem - k1y * zchunks;
-        double2 *base = a.W + col * a.ldw + (int64_t)(k1y * my) * a.nz + zc * TZ;
-        switch (my) {
-        case 1: fft3_x_load_y<1, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 2: fft3_x_load_y<2, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 3: fft3_x_load_y<3, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 4: fft3_x_load_y<4, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 5: fft3_x_load_y<5, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 6: fft3_x_load_y<6, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 7: fft3_x_load_y<7, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 8: fft3_x_load_y<8, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 10: fft3_x_load_y<10, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 12: fft3_x_load_y<12, NX, TZ, NT>(a, base, S, P, tid); break;
-        default: fft3_x_load_y<16, NX, TZ, NT>(a, base, S, P, tid); break;
+        const int64_t toff = (int64_t)(k1y * my) * a.nz + zc * TZ;
+        fft3_x_tile<NX, TZ, NT, false>(a, a.W + col * a.ldw + toff, a.kin_yz + toff, S, twx_s, kinx_s, tid);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The persistent pipeline: ONE launch applies T + V_loc to all `ncol` columns.  Work items (phase, column, tile)
+// are handed out in queue order by an atomic counter; the queue is built from "super-steps": super-step s holds the
+// fwd items of column s, the x items of column s-1 and the inv items of column s-2, interleaved by `pattern`
+// (one entry per item of a super-step: phase << 28 | tile).  An x item of column c needs ALL fwd items of c, an inv
+// item ALL x items of c: per-column completion counters `done[phase*ncol + c]`, waited on by a spin (dependencies
+// always sit earlier in the queue, and a CTA never waits while holding an earlier unfinished item, so the smallest
+// unfinished item always makes progress: no co-residency assumption, no deadlock).  About three columns of k-space
+// are in flight, so the k-space written by fwd is still in L2 when x and inv read it.
+// CTA = 256 threads: the x program runs one tile with all of them; the fwd and inv programs run TWO tiles side by side
+// (two 128-thread groups with their own named barrier and their own half of the shared memory).
+struct PipeArgs {
+    int32_t *head;           // queue position counter (zeroed before the launch)
+    int32_t *done;           // [3][ncol] finished items per (phase, column) (zeroed before the launch)
+    const uint32_t *pattern; // item order inside one super-step
+    int32_t npattern;
+    int32_t n_fwd, n_x, n_inv;   // items per column and phase
+    int32_t zchunks;             // nz / TZ
+};
+
+template <int N, int R2Y> struct PipeCfg {
+    static constexpr int TZ = XCfg<N>::TZ;
+    static constexpr size_t smem(int my)
+    {
+        const size_t zy = 2 * ZyCfg<N, R2Y>::SMEM_FWD;
+        const size_t x = (size_t)N * (my * TZ + 1) * sizeof(double2);
+        return zy > x ? zy : x;
+    }
+};
+
+__device__ __forceinline__ void pipe_wait(const int32_t *cnt, int want)
+{
+    while (*((const volatile int32_t *)cnt) < want) __nanosleep(64);
+    __threadfence();
+}
+
+template <int N, int R2Y>
+__global__ void __launch_bounds__(256, 2) fft3_pipeline_kernel(Fft3Args a, PipeArgs q)
+{
+    using C = ZyCfg<N, R2Y>;
+    constexpr int TZ = XCfg<N>::TZ, NT = 256, NH = 128;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2 *S = reinterpret_cast<double2 *>(smem_raw);
+    __shared__ double2 twz_s[C::NTWZ];           // z twiddles = x twiddles (cubic in x and z)
+    __shared__ double kinx_s[N];
+    __shared__ double2 twy_s[2][R2Y];
+    __shared__ int32_t next_item;
+    const int tid = threadIdx.x, half = tid >> 7, htid = tid & (NH - 1);
+    const int my = a.my;
+    fft3_x_tables<N, NT>(a, twz_s, kinx_s, tid);
+    if (tid == 0) next_item = atomicAdd(q.head, 1);
+    __syncthreads();
+    const int64_t total = (int64_t)(a.ncol + 2) * q.npattern;
+    for (;;) {
+        const int item = next_item;
+        __syncthreads();                                          // everyone has read next_item
+        if (item >= total) break;
+        if (tid == 0) next_item = atomicAdd(q.head, 1);           // its latency hides behind this item
+        const int s = item / q.npattern;
+        const uint32_t e = q.pattern[item - s * q.npattern];
+        const int ph = (int)(e >> 28), t = (int)(e & 0x0fffffffu);
+        const int col = s - ph;
+        if (col < 0 || col >= a.ncol) { __syncthreads(); continue; }
+        if (ph == 0) {
+            // two fwd tiles side by side: tile u = 2t + half -> (x, n2y) = (u / my, u % my)
+            const int u = 2 * t + half, x = u / my, n2y = u - x * my;
+            if (htid < R2Y) twy_s[half][htid] = a.twy[n2y * htid];
+            group_sync(1 + half, NH);
+            fft3_fwd_tile<N, R2Y, NH>(a.X + (int64_t)col * a.ldx + (int64_t)x * a.ny * N, a.W + (int64_t)col * a.ldw + (int64_t)x * a.ny * N,
+                                      my, n2y, S + half * C::TILE, twz_s, twy_s[half], htid, 1 + half);
+        } else if (ph == 1) {
+            if (tid == 0) pipe_wait(q.done + col, q.n_fwd);
+            __syncthreads();
+            const int k1y = t / q.zchunks, zc = t - k1y * q.zchunks;
+            const int64_t toff = (int64_t)(k1y * my) * a.nz + zc * TZ;
+            fft3_x_tile<N, TZ, NT, true>(a, a.W + (int64_t)col * a.ldw + toff, a.kin_yz + toff, S, twz_s, kinx_s, tid);
+        } else {
+            if (tid == 0) pipe_wait(q.done + a.ncol + col, q.n_x);
+            __syncthreads();
+            const int u = 2 * t + half, x = u / my, n2y = u - x * my;
+            if (htid < R2Y) twy_s[half][htid] = a.twy[n2y * htid];
+            const int64_t po = (int64_t)x * a.ny * N;
+            double2 *Sh = S + half * C::TILE;
+            fft3_issue_w_tile<N, R2Y, NH>(a.W + (int64_t)col * a.ldw + po, my, n2y, Sh, htid);     // cp.async.cg: L2 only
+            cp_async_commit();
+            cp_async_wait<0>();
+            group_sync(1 + half, NH);
+            fft3_inv_stages_12<N, R2Y, NH>(Sh, twy_s[half], htid, 1 + half);
+            group_sync(1 + half, NH);
+            fft3_inv_stage_3<N, R2Y, NH, false>(Sh, twz_s, nullptr, a.X + (int64_t)col * a.ldx + po, a.vloc + po,
+                                                a.HX + (int64_t)col * a.ldhx + po, my, n2y, htid);
         }
-        __syncthreads();
-        // x stage A: radix-MX over n1 (x = n1*16 + n2), twiddle, in place
-        for (int item = tid; item < lines * 16; item += NT) {
-            const int n2 = item & 15, line = item >> 4;
-            double2 *p = S + n2 * P + line;
-            double re[MX], im[MX];
-#pragma unroll
-            for (int n1 = 0; n1 < MX; ++n1) { const double2 v = p[n1 * 16 * P]; re[n1] = v.x; im[n1] = v.y; }
-            Dft<MX>::run(re, im);
-#pragma unroll
-            for (int k = 1; k < MX; ++k) { const double2 w = twx_s[(k - 1) * 16 + n2]; tw_mul(re[k], im[k], w.x, -w.y); }
-#pragma unroll
-            for (int k = 0; k < MX; ++k) p[k * 16 * P] = make_double2(re[k], im[k]);
+        __syncthreads();                                          // all stores of this item are issued
+        if (tid == 0) {
+            __threadfence();
+            if (ph < 2) atomicAdd(q.done + ph * a.ncol + col, 1);
         }
-        __syncthreads();
-        // x stage B (radix-16 over n2) -> frequency kx = k1 + MX*k2; kinetic factor; inverse stage B'
-        for (int item = tid; item < lines * MX; item += NT) {
-            const int line = item % lines, k1 = item / lines;
-            double2 *p = S + k1 * 16 * P + line;
-            double br[16], bi[16];
-#pragma unroll
-            for (int t = 0; t < 16; ++t) { const double2 v = p[t * P]; br[t] = v.x; bi[t] = v.y; }
-            Dft<16>::run(br, bi);
-            const int jy = line / TZ, z = line - jy * TZ;
-            const double tin = __ldg(a.kin_yz + (int64_t)(k1y * my + jy) * a.nz + zc * TZ + z);
-#pragma unroll
-            for (int k2 = 0; k2 < 16; ++k2) {
-                const double f = kinx_s[k1 + MX * k2] + tin;
-                br[k2] *= f; bi[k2] *= f;
-            }
-            Dft<16>::run(bi, br);                  // swapped domain from here on
-#pragma unroll
-            for (int t = 0; t < 16; ++t) p[t * P] = make_double2(br[t], bi[t]);
-        }
-        __syncthreads();
-        // x inverse stage A': conj twiddle, radix-MX over k1 -> x = n1*16 + n2
-        for (int item = tid; item < lines * 16; item += NT) {
-            const int n2 = item & 15, line = item >> 4;
-            double2 *p = S + n2 * P + line;
-            double re[MX], im[MX];
-#pragma unroll
-            for (int k = 0; k < MX; ++k) { const double2 v = p[k * 16 * P]; re[k] = v.x; im[k] = v.y; }
-#pragma unroll
-            for (int k = 1; k < MX; ++k) { const double2 w = twx_s[(k - 1) * 16 + n2]; tw_mul(im[k], re[k], w.x, -w.y); }
-            Dft<MX>::run(im, re);
-#pragma unroll
-            for (int n1 = 0; n1 < MX; ++n1) p[n1 * 16 * P] = make_double2(re[n1], im[n1]);
-        }
-        __syncthreads();
-        switch (my) {
-        case 1: fft3_x_store_y<1, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 2: fft3_x_store_y<2, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 3: fft3_x_store_y<3, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 4: fft3_x_store_y<4, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 5: fft3_x_store_y<5, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 6: fft3_x_store_y<6, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 7: fft3_x_store_y<7, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 8: fft3_x_store_y<8, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 10: fft3_x_store_y<10, NX, TZ, NT>(a, base, S, P, tid); break;
-        case 12: fft3_x_store_y<12, NX, TZ, NT>(a, base, S, P, tid); break;
-        default: fft3_x_store_y<16, NX, TZ, NT>(a, base, S, P, tid); break;
-        }
-        __syncthreads();
     }
 }
 

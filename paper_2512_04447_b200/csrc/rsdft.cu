@@ -114,6 +114,10 @@ struct rsdft_plan {
     // apply_h batching
     int batch = 0;                // columns per kernel sequence
     int user_batch = 0;
+    int pipeline = 0;             // 1: persistent FFT pipeline kernel where available (rsdft_plan_set_pipeline)
+    DevBuf<uint32_t> pipe_pattern;
+    DevBuf<int32_t> pipe_counters;
+    int pipe_key = -1, pipe_npattern = 0;
 
     // gram workspace
     DevBuf<double2> gram_work;
@@ -354,6 +358,17 @@ int build_spheres(rsdft_plan *P, const rsdft_atoms_t *atoms, const rsdft_project
     return RSDFT_OK;
 }
 
+// first-stage radix of an axis: 16 when it divides N, else 12 (fft3_kernels.cuh); 0 = length not supported
+int first_radix(int N)
+{
+    if (rsdft::radix16_ok(N)) return 16;
+    if (N % 12 == 0) {
+        const int M = N / 12;
+        return (M == 1 || M == 2 || M == 3 || M == 5 || M == 6 || M == 7 || M == 10 || M == 12) ? 12 : 0;
+    }
+    return 0;
+}
+
 int build_fft_tables(rsdft_plan *P)
 {
     for (int ax = 0; ax < 3; ++ax) {
@@ -373,12 +388,14 @@ int build_fft_tables(rsdft_plan *P)
     };
     std::vector<double> kx(P->n[0]), kyz((size_t)P->n[1] * P->n[2]);
     for (int i = 0; i < P->n[0]; ++i) kx[i] = (double)(t_axis(0, i) * inv_ng);
-    // k-space positions are permuted by the in-place transforms: y row r = k1*My + k2 holds ky = k1 + 16*k2
-    // ("16-first"), z position p = k1*16 + k2 holds kz = k1 + Mz*k2 ("M-first"); x is indexed naturally.
-    const int My = P->n[1] / 16, Mz = P->n[2] / 16;
+    // k-space positions are permuted by the in-place transforms (N = R2*M, R2 = 16 or 12): y row r = k1*My + k2
+    // holds ky = k1 + R2y*k2 ("R2-first"), z position p = k1*R2z + k2 holds kz = k1 + Mz*k2 ("M-first"); x is
+    // indexed naturally.
+    const int R2y = first_radix(P->n[1]), R2z = first_radix(P->n[2]);
+    const int My = P->n[1] / R2y, Mz = P->n[2] / R2z;
     for (int r = 0; r < P->n[1]; ++r)
         for (int p = 0; p < P->n[2]; ++p) {
-            const int ky = r / My + 16 * (r % My), kz = p / 16 + Mz * (p % 16);
+            const int ky = r / My + R2y * (r % My), kz = p / R2z + Mz * (p % R2z);
             kyz[(size_t)r * P->n[2] + p] = (double)((t_axis(1, ky) + t_axis(2, kz)) * inv_ng);
         }
     RS_CUDA(P->kin_x.upload(kx));
@@ -399,14 +416,22 @@ using namespace rsdft;
 
 #define RS_DISPATCH_N(ERR_, N_, FN_, ...)                                    \
     switch (N_) {                                                            \
+    case 12: ERR_ = FN_<12>(__VA_ARGS__); break;                             \
     case 16: ERR_ = FN_<16>(__VA_ARGS__); break;                             \
+    case 24: ERR_ = FN_<24>(__VA_ARGS__); break;                             \
     case 32: ERR_ = FN_<32>(__VA_ARGS__); break;                             \
+    case 36: ERR_ = FN_<36>(__VA_ARGS__); break;                             \
     case 48: ERR_ = FN_<48>(__VA_ARGS__); break;                             \
+    case 60: ERR_ = FN_<60>(__VA_ARGS__); break;                             \
     case 64: ERR_ = FN_<64>(__VA_ARGS__); break;                             \
+    case 72: ERR_ = FN_<72>(__VA_ARGS__); break;                             \
     case 80: ERR_ = FN_<80>(__VA_ARGS__); break;                             \
+    case 84: ERR_ = FN_<84>(__VA_ARGS__); break;                             \
     case 96: ERR_ = FN_<96>(__VA_ARGS__); break;                             \
     case 112: ERR_ = FN_<112>(__VA_ARGS__); break;                           \
+    case 120: ERR_ = FN_<120>(__VA_ARGS__); break;                           \
     case 128: ERR_ = FN_<128>(__VA_ARGS__); break;                           \
+    case 144: ERR_ = FN_<144>(__VA_ARGS__); break;                           \
     case 160: ERR_ = FN_<160>(__VA_ARGS__); break;                           \
     case 192: ERR_ = FN_<192>(__VA_ARGS__); break;                           \
     case 256: ERR_ = FN_<256>(__VA_ARGS__); break;                           \
@@ -419,11 +444,11 @@ inline int occ_by_smem(size_t smem, int cap)
     return (int)std::max<size_t>(1, std::min<size_t>((size_t)cap, (size_t)(228 * 1024) / (smem + 2048)));
 }
 
-template <int NZ>
-cudaError_t launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
+template <int NZ, int R2Y>
+cudaError_t launch_fwd_zy_r(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    auto k = fft3_fwd_zy_kernel<NZ, 4>;
-    const size_t smem = ZyCfg<NZ>::SMEM_FWD;
+    auto k = fft3_fwd_zy_kernel<NZ, R2Y, 4>;
+    const size_t smem = ZyCfg<NZ, R2Y>::SMEM_FWD;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     // G plane-walkers for each of the my row classes, two CTA generations of the resident set
@@ -433,10 +458,15 @@ cudaError_t launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
     return cudaSuccess;
 }
 template <int NZ>
-cudaError_t launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
+cudaError_t launch_fwd_zy(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    auto k = fft3_inv_yz_kernel<NZ, 2>;
-    const size_t smem = ZyCfg<NZ>::SMEM_INV;
+    return a.r2y == 16 ? launch_fwd_zy_r<NZ, 16>(a, sms, st) : launch_fwd_zy_r<NZ, 12>(a, sms, st);
+}
+template <int NZ, int R2Y>
+cudaError_t launch_inv_yz_r(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    auto k = fft3_inv_yz_kernel<NZ, R2Y, 2>;
+    const size_t smem = ZyCfg<NZ, R2Y>::SMEM_INV;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     // G x-plane walkers per row class; every walker runs over all columns of the batch
@@ -446,13 +476,18 @@ cudaError_t launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
     k<<<(int)(g * a.my), 128, smem, st>>>(a);
     return cudaSuccess;
 }
+template <int NZ>
+cudaError_t launch_inv_yz(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    return a.r2y == 16 ? launch_inv_yz_r<NZ, 16>(a, sms, st) : launch_inv_yz_r<NZ, 12>(a, sms, st);
+}
 
 template <int NX, int TZ, int NT, int MINB>
 cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
 {
     const size_t smem = (size_t)NX * (a.my * TZ + 1) * sizeof(double2);
-    if (smem + 4096 > 227 * 1024) return cudaErrorInvalidConfiguration;
-    const int64_t ntiles = (int64_t)a.ncol * 16 * (a.nz / TZ);
+    if (smem + 4096 > 227 * 1024 || a.nz % TZ != 0) return cudaErrorInvalidConfiguration;
+    const int64_t ntiles = (int64_t)a.ncol * a.r2y * (a.nz / TZ);
     auto k = fft3_x_kernel<NX, TZ, NT, MINB>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -464,11 +499,35 @@ cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
 template <int NX>
 cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 {
-    // the tile is NX x (my*TZ) elements: fall back to narrower z chunks when a large ny makes it too big
-    auto fits = [&](int tz) { return (size_t)NX * (a.my * tz + 1) * sizeof(double2) + 4096 <= (size_t)227 * 1024; };
+    // the tile is NX x (my*TZ) elements: fall back to narrower z chunks when a large ny makes it too big or
+    // when nz is not a multiple of the preferred chunk (nz = 12*M with odd M)
+    auto fits = [&](int tz) { return a.nz % tz == 0 && (size_t)NX * (a.my * tz + 1) * sizeof(double2) + 4096 <= (size_t)227 * 1024; };
     if (fits(XCfg<NX>::TZ)) return launch_x_cfg<NX, XCfg<NX>::TZ, XCfg<NX>::NT, XCfg<NX>::MINB>(a, sms, st);
     if (fits(4)) return launch_x_cfg<NX, 4, 256, 1>(a, sms, st);
     return launch_x_cfg<NX, 2, 256, 1>(a, sms, st);
+}
+
+// the persistent pipeline kernel exists for cubic grids of these lengths (the shapes of the five configs and of
+// the paper's two grids); everything else runs the three-kernel path
+template <int N>
+cudaError_t launch_pipeline(const Fft3Args &a, const PipeArgs &q, int sms, cudaStream_t st)
+{
+    constexpr int R2 = Axis<N>::R2;
+    auto k = fft3_pipeline_kernel<N, R2>;
+    const size_t smem = PipeCfg<N, R2>::smem(a.my);
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int64_t total = (int64_t)(a.ncol + 2) * q.npattern;
+    k<<<(int)std::min<int64_t>(total, (int64_t)sms * 2), 256, smem, st>>>(a, q);
+    return cudaSuccess;
+}
+inline bool pipeline_available(const int n[3])
+{
+    if (n[0] != n[1] || n[1] != n[2]) return false;
+    switch (n[0]) {
+    case 48: case 60: case 64: case 80: case 96: case 112: case 128: return true;
+    default: return false;
+    }
 }
 
 template <int MT>
@@ -513,24 +572,46 @@ int default_batch(const rsdft_plan *P)
     return (int)std::max<int64_t>(1, std::min<int64_t>(b, 64));
 }
 
-// One batch of columns through the whole operator, on stream slot `slot`.
+Fft3Args fft3_args(const rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx)
+{
+    Fft3Args fa;
+    fa.X = X; fa.W = HX; fa.HX = HX; fa.ldx = ldx; fa.ldw = ldhx; fa.ldhx = ldhx;
+    fa.ncol = nb; fa.nx = P->n[0]; fa.ny = P->n[1]; fa.nz = P->n[2];
+    fa.r2y = first_radix(P->n[1]); fa.my = P->n[1] / fa.r2y;
+    fa.twx = P->tw[0].p; fa.twy = P->tw[1].p; fa.twz = P->tw[2].p;
+    fa.kin_x = P->kin_x.p; fa.kin_yz = P->kin_yz.p; fa.vloc = P->vloc.p;
+    return fa;
+}
+
+void launch_project(rsdft_plan *P, const SphereTables &tabs, int nb, const double2 *X, int64_t ldx, double2 *pp, double2 *pq, cudaStream_t st)
+{
+    if (P->maxproj <= 8) launch_project_mt<1>(tabs, X, ldx, nb, P->dV, pp, P->num_sms, st);
+    else launch_project_mt<2>(tabs, X, ldx, nb, P->dV, pp, P->num_sms, st);
+    combine_kernel<<<dim3(P->natom, (nb + NL_CCOLS - 1) / NL_CCOLS), 128, 0, st>>>(tabs, pp, nb, pq);
+    P->last_launches += 2;
+}
+
+void launch_scatter(rsdft_plan *P, const SphereTables &tabs, int nb, const double2 *pq, double2 *HX, int64_t ldhx, cudaStream_t st)
+{
+    for (int c = 0; c < P->ncolour; ++c) {
+        const int ch0 = P->colour_chunk_off[c], nlist = P->colour_chunk_off[c + 1] - ch0;
+        if (nlist == 0) continue;
+        if (P->maxproj <= 4) launch_scatter_np<4>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
+        else if (P->maxproj <= 9) launch_scatter_np<9>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
+        else launch_scatter_np<16>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
+        ++P->last_launches;
+    }
+}
+
+// One batch of columns through the whole operator, on stream slot `slot` (three FFT kernels per batch).
 int apply_h_batch(rsdft_plan *P, int slot, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
 {
-    const int Nx = P->n[0], Ny = P->n[1], Nz = P->n[2];
+    const int Nx = P->n[0], Nz = P->n[2];
     const bool nl = P->natom > 0 && P->total_pts > 0;
     const SphereTables tabs = sphere_tables(P);
     double2 *pp = P->pp[slot].p, *pq = P->pq[slot].p;
-    if (nl) {   // projections read the INPUT orbitals
-        if (P->maxproj <= 8) launch_project_mt<1>(tabs, X, ldx, nb, P->dV, pp, P->num_sms, st);
-        else launch_project_mt<2>(tabs, X, ldx, nb, P->dV, pp, P->num_sms, st);
-        combine_kernel<<<dim3(P->natom, (nb + NL_CCOLS - 1) / NL_CCOLS), 128, 0, st>>>(tabs, pp, nb, pq);
-        P->last_launches += 2;
-    }
-    Fft3Args fa;
-    fa.X = X; fa.W = HX; fa.HX = HX; fa.ldx = ldx; fa.ldw = ldhx; fa.ldhx = ldhx;
-    fa.ncol = nb; fa.nx = Nx; fa.ny = Ny; fa.nz = Nz; fa.my = Ny / 16;
-    fa.twx = P->tw[0].p; fa.twy = P->tw[1].p; fa.twz = P->tw[2].p;
-    fa.kin_x = P->kin_x.p; fa.kin_yz = P->kin_yz.p; fa.vloc = P->vloc.p;
+    if (nl) launch_project(P, tabs, nb, X, ldx, pp, pq, st);    // projections read the INPUT orbitals
+    const Fft3Args fa = fft3_args(P, nb, X, ldx, HX, ldhx);
     cudaError_t ke = cudaSuccess;
     RS_DISPATCH_N(ke, Nz, launch_fwd_zy, fa, P->num_sms, st)              // z fwd, y fwd stage A:  X -> HX
     RS_CUDA(ke);
@@ -539,16 +620,83 @@ int apply_h_batch(rsdft_plan *P, int slot, int nb, const double2 *X, int64_t ldx
     RS_DISPATCH_N(ke, Nz, launch_inv_yz, fa, P->num_sms, st)              // y A', z inv, + v(r) psi(r)
     RS_CUDA(ke);
     P->last_launches += 3;
+    if (nl) launch_scatter(P, tabs, nb, pq, HX, ldhx, st);
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
+}
+
+// item order inside one super-step of the pipeline queue: the three phases interleaved in proportion
+int pipeline_pattern(rsdft_plan *P, const Fft3Args &fa, int tz, PipeArgs &q, cudaStream_t st)
+{
+    q.n_fwd = fa.nx * fa.my / 2;
+    q.zchunks = fa.nz / tz;
+    q.n_x = fa.r2y * q.zchunks;
+    q.n_inv = q.n_fwd;
+    const int key = fa.nx * 1024 + fa.my;
+    if (P->pipe_key != key) {
+        std::vector<std::pair<double, uint32_t>> items;
+        const int cnt[3] = {q.n_fwd, q.n_x, q.n_inv};
+        for (int ph = 0; ph < 3; ++ph)
+            for (int t = 0; t < cnt[ph]; ++t) items.push_back({(t + 0.5) / cnt[ph] + 1e-9 * ph, ((uint32_t)ph << 28) | (uint32_t)t});
+        std::sort(items.begin(), items.end());
+        std::vector<uint32_t> pat(items.size());
+        for (size_t e = 0; e < items.size(); ++e) pat[e] = items[e].second;
+        RS_CUDA(P->pipe_pattern.upload_async(pat, st));
+        P->pipe_key = key;
+        P->pipe_npattern = (int)pat.size();
+    }
+    q.pattern = P->pipe_pattern.p;
+    q.npattern = P->pipe_npattern;
+    return RSDFT_OK;
+}
+
+// All columns through ONE persistent FFT kernel (k-space handed over through L2); the projections of every batch
+// run before it, the scatter-adds after it, everything on the caller's stream.
+int apply_h_pipeline(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, int batch, cudaStream_t st)
+{
+    const bool nl = P->natom > 0 && P->total_pts > 0;
+    const SphereTables tabs = sphere_tables(P);
+    const size_t qstride = (size_t)P->natom * P->maxproj * batch;
+    const int nbatches = (ncol + batch - 1) / batch;
     if (nl) {
-        for (int c = 0; c < P->ncolour; ++c) {
-            const int ch0 = P->colour_chunk_off[c], nlist = P->colour_chunk_off[c + 1] - ch0;
-            if (nlist == 0) continue;
-            if (P->maxproj <= 4) launch_scatter_np<4>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
-            else if (P->maxproj <= 9) launch_scatter_np<9>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
-            else launch_scatter_np<16>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
-            ++P->last_launches;
+        RS_CUDA(P->pp[0].ensure((size_t)P->nchunks * P->maxproj * batch));
+        RS_CUDA(P->pq[0].ensure(qstride * nbatches));
+        for (int k = 0; k < nbatches; ++k) {
+            const int c0 = k * batch, nb = std::min(batch, ncol - c0);
+            launch_project(P, tabs, nb, X + (int64_t)c0 * ldx, ldx, P->pp[0].p, P->pq[0].p + qstride * k, st);
         }
     }
+    const Fft3Args fa = fft3_args(P, ncol, X, ldx, HX, ldhx);
+    PipeArgs q;
+    int tz = 0;
+    switch (P->n[0]) {
+    case 48: tz = XCfg<48>::TZ; break;  case 60: tz = XCfg<60>::TZ; break;  case 64: tz = XCfg<64>::TZ; break;
+    case 80: tz = XCfg<80>::TZ; break;  case 96: tz = XCfg<96>::TZ; break;  case 112: tz = XCfg<112>::TZ; break;
+    default: tz = XCfg<128>::TZ; break;
+    }
+    if (int rc = pipeline_pattern(P, fa, tz, q, st)) return rc;
+    RS_CUDA(P->pipe_counters.ensure((size_t)3 * ncol + 4));
+    RS_CUDA(cudaMemsetAsync(P->pipe_counters.p, 0, ((size_t)3 * ncol + 4) * sizeof(int32_t), st));
+    q.head = P->pipe_counters.p;
+    q.done = P->pipe_counters.p + 4;
+    cudaError_t ke = cudaSuccess;
+    switch (P->n[0]) {
+    case 48: ke = launch_pipeline<48>(fa, q, P->num_sms, st); break;
+    case 60: ke = launch_pipeline<60>(fa, q, P->num_sms, st); break;
+    case 64: ke = launch_pipeline<64>(fa, q, P->num_sms, st); break;
+    case 80: ke = launch_pipeline<80>(fa, q, P->num_sms, st); break;
+    case 96: ke = launch_pipeline<96>(fa, q, P->num_sms, st); break;
+    case 112: ke = launch_pipeline<112>(fa, q, P->num_sms, st); break;
+    case 128: ke = launch_pipeline<128>(fa, q, P->num_sms, st); break;
+    default: ke = cudaErrorInvalidValue; break;
+    }
+    RS_CUDA(ke);
+    ++P->last_launches;
+    if (nl)
+        for (int k = 0; k < nbatches; ++k) {
+            const int c0 = k * batch, nb = std::min(batch, ncol - c0);
+            launch_scatter(P, tabs, nb, P->pq[0].p + qstride * k, HX + (int64_t)c0 * ldhx, ldhx, st);
+        }
     RS_CUDA(cudaGetLastError());
     return RSDFT_OK;
 }
@@ -557,6 +705,7 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
 {
     const int batch = P->user_batch > 0 ? P->user_batch : default_batch(P);
     P->batch = batch;
+    if (P->pipeline && pipeline_available(P->n)) return apply_h_pipeline(P, ncol, X, ldx, HX, ldhx, batch, st);
     const int nbatches = (ncol + batch - 1) / batch;
     const int ns = std::max(1, std::min(std::min(P->nstreams, (int)rsdft_plan::MAX_STREAMS), nbatches));
     if (P->natom > 0 && P->total_pts > 0)
@@ -740,10 +889,9 @@ int rsdft_plan_create(const rsdft_grid_t *grid, const rsdft_box_t *box, const rs
     for (int a = 0; a < 3; ++a) {
         const int N = grid->n[a];
         if (N <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_plan_create: grid length <= 0");
-        const int M = N / 16;
-        if (N % 16 != 0 || !(M <= 8 || M == 10 || M == 12 || M == 16))
+        if (first_radix(N) == 0)
             return fail(RSDFT_UNSUPPORTED, "rsdft_plan_create: grid length " + std::to_string(N) +
-                                               " not in {16,32,48,64,80,96,112,128,160,192,256}");
+                                               " not in {12,16,24,32,36,48,60,64,72,80,84,96,112,120,128,144,160,192,256}");
         if (!(box->len[a] > 0.0) || !std::isfinite(box->len[a]))
             return fail(RSDFT_UNSUPPORTED, "rsdft_plan_create: box length must be positive and finite");
     }
@@ -813,6 +961,13 @@ int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols)
 {
     if (!plan || batch_cols < 0 || batch_cols > 65535) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_batch: bad argument");
     plan->user_batch = batch_cols;
+    return RSDFT_OK;
+}
+
+int rsdft_plan_set_pipeline(rsdft_plan_t *plan, int32_t mode)
+{
+    if (!plan || (mode != 0 && mode != 1)) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_pipeline: mode must be 0 or 1");
+    plan->pipeline = mode;
     return RSDFT_OK;
 }
 

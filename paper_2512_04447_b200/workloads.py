@@ -28,6 +28,12 @@ CONFIGS = {
             depth=4.0, width=1.0, nproj=9, rc=2.2),
     4: dict(name="cfg4-large128", n=128, L=26.0, m=512, seed=4, atoms="minsep", natom=256,
             depth=4.0, width=1.0, nproj=9, rc=2.2, minsep=3.0),
+    # the paper's own benchmark shapes: diamond-216 on 60^3 with N = 436 orbitals and W-128 on 80^3
+    # with N = 901, with the synthetic potentials/projectors of configs 2 and 3 (the ONCV files are not available)
+    5: dict(name="paper-diamond60", n=60, L=20.22, m=436, seed=5, atoms="diamond", natom=216,
+            depth=3.0, width=0.8, nproj=4, rc=1.4),
+    6: dict(name="paper-tungsten80", n=80, L=23.92, m=901, seed=6, atoms="bcc", natom=128,
+            depth=4.0, width=1.0, nproj=9, rc=2.2),
 }
 
 

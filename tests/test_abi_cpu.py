@@ -52,7 +52,7 @@ def test_plan_create_rejects_bad_arguments(lib):
         rsdft.rsdft_plan_create((20, 16, 16), (10.0, 10.0, 10.0))
     assert e.value.code == rsdft.RSDFT_UNSUPPORTED and "20" in str(e.value)
     with pytest.raises(rsdft.RsdftError) as e:
-        rsdft.rsdft_plan_create((16, 16, 144), (10.0, 10.0, 10.0))
+        rsdft.rsdft_plan_create((16, 16, 176), (10.0, 10.0, 10.0))      # 16 * 11 and not a multiple of 12
     assert e.value.code == rsdft.RSDFT_UNSUPPORTED
     with pytest.raises(rsdft.RsdftError) as e:
         rsdft.rsdft_plan_create((16, 16, 16), (10.0, -1.0, 10.0))

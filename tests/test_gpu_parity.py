@@ -88,7 +88,7 @@ def test_apply_h_only_x_block_config0(env):
 
 
 # ------------------------------------------------------------------ every supported length on every axis
-@pytest.mark.parametrize("N", [16, 32, 48, 64, 80, 96, 112, 128, 160, 192, 256])
+@pytest.mark.parametrize("N", [12, 16, 24, 32, 36, 48, 60, 64, 72, 80, 84, 96, 112, 120, 128, 144, 160, 192, 256])
 @pytest.mark.parametrize("axis", [0, 1, 2])
 def test_kinetic_every_length_every_axis(env, N, axis):
     torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
@@ -113,6 +113,51 @@ def test_kinetic_every_length_every_axis(env, N, axis):
     # round-off in the empty Fourier modes is amplified by their own t(k): scale by max_k t(k)
     tmax = 0.5 * sum((np.pi * n[a] / L[a]) ** 2 for a in range(3))
     assert np.max(np.abs(Tpw - lam * pw.cpu().numpy())) <= 1e-13 * tmax
+
+
+@pytest.mark.parametrize("n3", [(60, 36, 24), (12, 60, 84), (24, 16, 60), (60, 60, 60)])
+def test_lengths_with_first_radix_12(env, n3):
+    """Grids whose lengths are 12*M (the paper's 60^3 among them), mixed with 16*M ones, with projectors."""
+    oracle, rsdft, wl = env["oracle"], env["rsdft"], env["wl"]
+    L = tuple(0.23 * v for v in n3)
+    system = wl.small_system(n=n3, L=L, natom=3, seed=4, nproj=9, rc=1.3)
+    ng = int(np.prod(n3))
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(ng, range(3), 15, 0, device="cuda")
+    HX = gpu_apply(env, plan, X)
+    assert col_err(HX.cpu().numpy(), oracle.apply_h(system, X.cpu().numpy())) <= TOL
+    plan.close()
+
+
+@pytest.mark.parametrize("N,ncol", [(48, 13), (60, 9), (64, 7), (80, 5), (96, 7), (112, 4), (128, 3)])
+def test_pipeline_kernel_matches_three_kernel_path(env, N, ncol):
+    """rsdft_plan_set_pipeline(1): the persistent FFT kernel (work queue + per-column completion counters) gives the
+    same bits as the three-kernel path, on a caller's side stream, with overlapping projector spheres; and both match
+    the oracle on sampled columns."""
+    torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
+    L = (0.22 * N,) * 3
+    system = wl.small_system(n=(N, N, N), L=L, natom=6, seed=N, nproj=4, rc=1.8)
+    ng = N ** 3
+    plan = rsdft.plan_from_system(system)
+    X = wl.orbital_block(ng, range(ncol), 31, 0, device="cuda", ld=ng + 16)
+    ref = gpu_apply(env, plan, X)
+    rsdft.rsdft_plan_set_pipeline(plan, 1)
+    side = torch.cuda.Stream()
+    outs = []
+    for batch in (0, 2):
+        rsdft.rsdft_plan_set_batch(plan, batch)
+        with torch.cuda.stream(side):
+            HX = torch.full_like(X, float("nan"))
+            rsdft.rsdft_apply_h(plan, X, HX)
+            outs.append(HX.clone())
+        side.synchronize()
+    for o in outs:
+        assert torch.equal(torch.view_as_real(o[:, :ng]), torch.view_as_real(ref[:, :ng]))
+        assert bool(torch.isnan(o[:, ng:].real).all())
+    cols = [0, ncol - 1]
+    assert col_err(outs[0][cols, :ng].cpu().numpy(), oracle.apply_h(system, X[cols, :ng].cpu().numpy())) <= TOL
+    assert rsdft.rsdft_plan_info(plan)["last_launches"] >= 1
+    plan.close()
 
 
 # ------------------------------------------------------------------ degenerate / ragged inputs
@@ -209,10 +254,13 @@ def test_error_paths_on_device(env):
         rsdft.rsdft_apply_h(plan, X, X)                                   # aliasing
     assert e.value.code == rsdft.RSDFT_INVALID_ARG and "overlap" in str(e.value)
     short = torch.zeros((2, 4000), dtype=torch.complex128, device="cuda")
-    with pytest.raises(rsdft.RsdftError):
-        rsdft.rsdft_apply_h(plan, short, torch.zeros_like(short))         # ld < Ng
-    with pytest.raises(rsdft.RsdftError):
+    with pytest.raises(ValueError):
+        rsdft.rsdft_apply_h(plan, short, torch.zeros_like(short))         # ld < Ng: caught by the binding
+    with pytest.raises(ValueError):
         rsdft.rsdft_subspace_gram(plan, short, short)
+    lib0 = rsdft.load()                                                   # ... and by the C ABI itself
+    assert lib0.rsdft_apply_h(plan.handle, 2, X.data_ptr(), 4000, X.data_ptr() + 2 * 4096 * 16, 4096, None) == rsdft.RSDFT_INVALID_ARG
+    assert lib0.rsdft_subspace_gram(plan.handle, 2, X.data_ptr(), 4000, X.data_ptr(), 4000, X.data_ptr(), X.data_ptr(), 2, None) == rsdft.RSDFT_INVALID_ARG
     with pytest.raises(ValueError):
         rsdft.rsdft_apply_h(plan, X.cpu(), X)                             # host tensor
     lib = rsdft.load()
@@ -333,9 +381,10 @@ def test_binding_rejects_wrong_output_tensors(env):
 
 
 # ------------------------------------------------------------------ BASELINE.json full sizes, bench.py's launch configuration
-@pytest.mark.parametrize("cfg", [2, 3, 4])
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5, 6])
 def test_full_size_block_step_sampled_parity(env, cfg):
-    """configs[2..4] at full size (n = 3m columns, whole block resident in HBM), the library's default
+    """configs[2..4] (and the paper's own shapes, workloads.CONFIGS[5, 6]: diamond-216 on 60^3 with 436 orbitals, W-128 on
+    80^3 with 901) at full size (n = 3m columns, whole block resident in HBM), the library's default
     batching/streams, i.e. exactly what bench.py times.  The oracle recomputes a seeded sample of columns
     spread over X, W, P (HX element by element) and the matching |C| x |C| sub-blocks of H_sub and S_sub
     over the full grid; the rest of the matrices is checked through invariants that hold at any size."""
