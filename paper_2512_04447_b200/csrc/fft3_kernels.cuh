@@ -507,6 +507,7 @@ struct PipeArgs {
     int32_t npattern;
     int32_t n_fwd, n_x, n_inv;   // items per column and phase
     int32_t zchunks;             // nz / TZ
+    int32_t lag_x, lag_inv;      // super-step s holds fwd(s), x(s - lag_x), inv(s - lag_inv)
 };
 
 template <int N, int R2Y> struct PipeCfg {
@@ -541,7 +542,7 @@ __global__ void __launch_bounds__(256, 2) fft3_pipeline_kernel(Fft3Args a, PipeA
     fft3_x_tables<N, NT>(a, twz_s, kinx_s, tid);
     if (tid == 0) next_item = atomicAdd(q.head, 1);
     __syncthreads();
-    const int64_t total = (int64_t)(a.ncol + 2) * q.npattern;
+    const int64_t total = (int64_t)(a.ncol + q.lag_inv) * q.npattern;
     for (;;) {
         const int item = next_item;
         __syncthreads();                                          // everyone has read next_item
@@ -550,7 +551,7 @@ __global__ void __launch_bounds__(256, 2) fft3_pipeline_kernel(Fft3Args a, PipeA
         const int s = item / q.npattern;
         const uint32_t e = q.pattern[item - s * q.npattern];
         const int ph = (int)(e >> 28), t = (int)(e & 0x0fffffffu);
-        const int col = s - ph;
+        const int col = s - (ph == 0 ? 0 : (ph == 1 ? q.lag_x : q.lag_inv));
         if (col < 0 || col >= a.ncol) { __syncthreads(); continue; }
         if (ph == 0) {
             // two fwd tiles side by side: tile u = 2t + half -> (x, n2y) = (u / my, u % my)
