@@ -224,6 +224,12 @@ int rsdft_plan_set_gram_mode(rsdft_plan_t *plan, int32_t h_upper_only);
  * re-created on the next call that needs them.  Synchronises the device.  Errors: INVALID_ARG, CUDA. */
 int rsdft_plan_release_workspace(rsdft_plan_t *plan);
 
+/* Operand staging of the Gram kernel.  0 (default): per-thread 16-byte cp.async (LDGSTS).  1: one TMA bulk copy
+ * (cp.async.bulk + mbarrier, SASS UBLKCP) per 256-byte operand row and pipeline stage.  Bitwise identical results;
+ * measured 12 % slower at configs[2] (192 small bulk copies per stage cost more than they save), kept as the
+ * measured Blackwell-mechanism variant.  Errors: INVALID_ARG. */
+int rsdft_plan_set_gram_staging(rsdft_plan_t *plan, int32_t bulk);
+
 /* Destroys the plan and frees everything it owns (synchronises the device first). */
 int rsdft_plan_destroy(rsdft_plan_t *plan);
 

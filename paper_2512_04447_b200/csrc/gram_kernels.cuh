@@ -54,7 +54,9 @@ struct GramCfg {
     static constexpr size_t SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(double2);
 };
 
-template <int WGM, int WGN, int FA, int FB, int KC, int STAGES>
+// BULK: the operand rows of a stage (KC consecutive grid points of one column = 256 contiguous bytes) arrive by ONE
+// TMA bulk copy each (cp.async.bulk + mbarrier, SASS UBLKCP) instead of KC per-thread 16-byte cp.async (LDGSTS).
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES, bool BULK = false>
 __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
 {
     using Cfg = GramCfg<WGM, WGN, FA, FB, KC, STAGES>;
@@ -97,6 +99,32 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
         }
     };
 
+    // bulk variant: thread `row` < TM+TN owns one operand row; rows of columns >= n stay zero for the whole kernel
+    __shared__ uint64_t full_bar[STAGES];
+    const int my_col = tid < TM ? i0 + tid : j0 + tid - TM;
+    const bool my_row = BULK && tid < TM + TN && my_col < a.n;
+    const double2 *my_src = nullptr;
+    uint32_t stage_bytes = 0;
+    if (BULK) {
+        if (tid < TM + TN) my_src = (tid < TM ? Abase + (int64_t)my_col * lda : Bbase + (int64_t)my_col * ldb) + r0;
+        const int va = min(TM, max(0, a.n - i0)), vb = min(TN, max(0, a.n - j0));
+        stage_bytes = (uint32_t)((va + vb) * KC * sizeof(double2));
+        if (tid == 0) {
+#pragma unroll
+            for (int s = 0; s < STAGES; ++s) mbar_init(&full_bar[s], 1);
+            mbar_fence_init();
+        }
+        if (tid < TM + TN && !my_row)
+            for (int s = 0; s < STAGES; ++s)
+                for (int k = 0; k < KC; ++k) sm[(size_t)s * Cfg::STAGE_ELEMS + tid * PITCH + k] = make_double2(0.0, 0.0);
+        __syncthreads();
+    }
+    auto issue_bulk = [&](int stage, int chunk) {
+        if (tid == 0) mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
+        if (my_row)
+            bulk_g2s(sm + (size_t)stage * Cfg::STAGE_ELEMS + tid * PITCH, my_src + (int64_t)chunk * KC, KC * sizeof(double2), &full_bar[stage]);
+    };
+
     double cre[FA][FB][2], cim[FA][FB][2];
 #pragma unroll
     for (int x = 0; x < FA; ++x)
@@ -105,17 +133,18 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
 
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
-        if (s < nch) load_stage(s, s);
-        cp_async_commit();
+        if (s < nch) { if (BULK) issue_bulk(s, s); else load_stage(s, s); }
+        if (!BULK) cp_async_commit();
     }
 
     for (int ch = 0; ch < nch; ++ch) {
-        cp_async_wait<STAGES - 2>();
+        if (BULK) mbar_wait(&full_bar[ch % STAGES], (uint32_t)((ch / STAGES) & 1));
+        else cp_async_wait<STAGES - 2>();
         __syncthreads();
         {   // prefetch chunk ch+STAGES-1 into the stage consumed at iteration ch-1
             const int nx = ch + STAGES - 1;
-            if (nx < nch) load_stage(nx % STAGES, nx);
-            cp_async_commit();
+            if (nx < nch) { if (BULK) issue_bulk(nx % STAGES, nx); else load_stage(nx % STAGES, nx); }
+            if (!BULK) cp_async_commit();
         }
         const double2 *As = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + (wm * FA * 8 + g) * PITCH + t;
         const double2 *Bs = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + (TM + wn * FB * 8 + g) * PITCH + t;
@@ -141,7 +170,7 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
             }
         }
     }
-    cp_async_wait<0>();
+    if (!BULK) cp_async_wait<0>();
 
     // epilogue: C fragment element e of (x, y) is row g, column 2t+e of that 8x8 tile
     double2 *W = a.work + (int64_t)unit * (TM * TN);

@@ -172,6 +172,12 @@ __global__ void __launch_bounds__(128) combine_kernel(SphereTables t, const doub
     }
 }
 
+// One CTA = one sphere chunk (<= 128 points, one per thread) x every column of the launch: a thread keeps its point's
+// grid index and beta values in registers and walks the columns in groups of CG independent read-modify-writes, so
+// the beta table is read ONCE per (chunk, launch) however many columns the launch carries (with large tables --
+// configs 3, 4: 43 / 98 MB -- beta re-reads per column group used to outweigh the orbital traffic itself).
+// q of all columns sits in shared memory ([NP][ncol], dynamic).  blockIdx.y strides over the column groups when the
+// chunk list alone does not fill the GPU.
 template <int NP>
 __global__ void __launch_bounds__(NL_THREADS) scatter_kernel(SphereTables t, int32_t chunk0, const double2 *__restrict__ q,
                                                              int32_t ncol, double2 *__restrict__ HX, int64_t ldhx)
@@ -179,40 +185,51 @@ __global__ void __launch_bounds__(NL_THREADS) scatter_kernel(SphereTables t, int
     // chunk0: first chunk of one colour class (spheres of one class are pairwise disjoint, so the
     // read-modify-write below is race-free and the result is deterministic)
     constexpr int CG = NlCols<NP>::CGS;
+    extern __shared__ __align__(16) unsigned char nl_smem_raw[];
+    double2 *qs = reinterpret_cast<double2 *>(nl_smem_raw);          // [NP][ncol]
     const SphereChunk ch = t.chunks[chunk0 + blockIdx.x];
-    const int c0 = (gridDim.y - 1 - blockIdx.y) * CG;   // last columns first: the FFT before ended there (L2)
     const int a = ch.atom;
     const int64_t o = t.pt_off[a];
     const int npts = (int)(t.pt_off[a + 1] - o);
     const int np = t.nproj[a];
-    const int32_t *idx = t.idx + o + ch.start;
-    const double *beta = t.beta + t.beta_off[a] + ch.start;
-    const int nc = min(CG, ncol - c0);
-    __shared__ double2 qs[NP][CG];
-    for (int e = threadIdx.x; e < NP * CG; e += NL_THREADS) {
-        const int i = e / CG, c = e - i * CG;
-        qs[i][c] = (i < np && c < nc) ? q[((int64_t)a * t.maxproj + i) * ncol + c0 + c] : make_double2(0.0, 0.0);
+    for (int e = threadIdx.x; e < NP * ncol; e += NL_THREADS) {
+        const int i = e / ncol, c = e - i * ncol;
+        qs[e] = i < np ? q[((int64_t)a * t.maxproj + i) * ncol + c] : make_double2(0.0, 0.0);
+    }
+    const int s = threadIdx.x;
+    const bool live = s < ch.count;
+    int64_t g = 0;
+    double b[NP];
+#pragma unroll
+    for (int i = 0; i < NP; ++i) b[i] = 0.0;
+    if (live) {
+        g = t.idx[o + ch.start + s];
+        const double *beta = t.beta + t.beta_off[a] + ch.start + s;
+#pragma unroll
+        for (int i = 0; i < NP; ++i) b[i] = i < np ? __ldg(beta + (int64_t)i * npts) : 0.0;
     }
     __syncthreads();
-    double2 *hx = HX + (int64_t)c0 * ldhx;
-    for (int s = threadIdx.x; s < ch.count; s += NL_THREADS) {
-        const int64_t g = idx[s];
+    if (!live) return;
+    const int ngroups = (ncol + CG - 1) / CG;
+    for (int gy = ngroups - 1 - (int)blockIdx.y; gy >= 0; gy -= (int)gridDim.y) {   // last columns first: the FFT before ended there (L2)
+        const int c0 = gy * CG;
+        const int nc = min(CG, ncol - c0);
+        double2 *hx = HX + (int64_t)c0 * ldhx + g;
         double2 v[CG];
 #pragma unroll
-        for (int c = 0; c < CG; ++c) v[c] = c < nc ? hx[(int64_t)c * ldhx + g] : make_double2(0.0, 0.0);
+        for (int c = 0; c < CG; ++c) v[c] = c < nc ? hx[(int64_t)c * ldhx] : make_double2(0.0, 0.0);
 #pragma unroll
         for (int i = 0; i < NP; ++i) {
-            const double b = i < np ? __ldg(beta + (int64_t)i * npts + s) : 0.0;
 #pragma unroll
             for (int c = 0; c < CG; ++c) {
-                const double2 qq = qs[i][c];
-                v[c].x = fma(b, qq.x, v[c].x);
-                v[c].y = fma(b, qq.y, v[c].y);
+                const double2 qq = qs[i * ncol + min(c0 + c, ncol - 1)];
+                v[c].x = fma(b[i], qq.x, v[c].x);
+                v[c].y = fma(b[i], qq.y, v[c].y);
             }
         }
 #pragma unroll
         for (int c = 0; c < CG; ++c)
-            if (c < nc) hx[(int64_t)c * ldhx + g] = v[c];
+            if (c < nc) hx[(int64_t)c * ldhx] = v[c];
     }
 }
 

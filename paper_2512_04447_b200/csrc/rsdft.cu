@@ -127,6 +127,7 @@ struct rsdft_plan {
     std::vector<int> gram_panel_off;
     int gram_panel_n = -1;
     int gram_h_upper = 0;                             // 1: H_sub from its upper tiles, mirrored (rsdft_plan_set_gram_mode)
+    int gram_bulk = 0;                                // 1: TMA bulk-copy operand staging (rsdft_plan_set_gram_staging; measured slower)
 
     // host-buffer entry point
     DevBuf<double2> hostY, hostHY, hostHS;
@@ -547,10 +548,15 @@ void launch_project_mt(const SphereTables &t, const double2 *X, int64_t ldx, int
 }
 template <int NP>
 void launch_scatter_np(const SphereTables &t, int chunk0, int nlist, const double2 *q, int ncol, double2 *HX,
-                       int64_t ldhx, cudaStream_t st)
+                       int64_t ldhx, int sms, cudaStream_t st)
 {
     constexpr int CG = NlCols<NP>::CGS;
-    scatter_kernel<NP><<<dim3(nlist, (ncol + CG - 1) / CG), NL_THREADS, 0, st>>>(t, chunk0, q, ncol, HX, ldhx);
+    const int ngroups = (ncol + CG - 1) / CG;
+    // enough CTAs for ~4 per SM when the chunk list is short; otherwise one CTA per chunk walks all column groups
+    const int gy = std::max(1, std::min(ngroups, (4 * sms + nlist - 1) / nlist));
+    const size_t smem = (size_t)NP * ncol * sizeof(double2);
+    if (smem > 48 * 1024) cudaFuncSetAttribute(scatter_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    scatter_kernel<NP><<<dim3(nlist, gy), NL_THREADS, smem, st>>>(t, chunk0, q, ncol, HX, ldhx);
 }
 
 SphereTables sphere_tables(const rsdft_plan *P)
@@ -596,30 +602,33 @@ void launch_scatter(rsdft_plan *P, const SphereTables &tabs, int nb, const doubl
     for (int c = 0; c < P->ncolour; ++c) {
         const int ch0 = P->colour_chunk_off[c], nlist = P->colour_chunk_off[c + 1] - ch0;
         if (nlist == 0) continue;
-        if (P->maxproj <= 4) launch_scatter_np<4>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
-        else if (P->maxproj <= 9) launch_scatter_np<9>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
-        else launch_scatter_np<16>(tabs, ch0, nlist, pq, nb, HX, ldhx, st);
+        if (P->maxproj <= 4) launch_scatter_np<4>(tabs, ch0, nlist, pq, nb, HX, ldhx, P->num_sms, st);
+        else if (P->maxproj <= 9) launch_scatter_np<9>(tabs, ch0, nlist, pq, nb, HX, ldhx, P->num_sms, st);
+        else launch_scatter_np<16>(tabs, ch0, nlist, pq, nb, HX, ldhx, P->num_sms, st);
         ++P->last_launches;
     }
 }
 
-// One batch of columns through the whole operator, on stream slot `slot` (three FFT kernels per batch).
-int apply_h_batch(rsdft_plan *P, int slot, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
+// One unit of columns through the whole operator, on stream slot `slot`: the projections of all `nb` columns, then
+// the three FFT kernels per sub-batch of `fft_batch` columns, then the scatter-adds of all `nb` columns.
+int apply_h_batch(rsdft_plan *P, int slot, int nb, int fft_batch, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx, cudaStream_t st)
 {
     const int Nx = P->n[0], Nz = P->n[2];
     const bool nl = P->natom > 0 && P->total_pts > 0;
     const SphereTables tabs = sphere_tables(P);
     double2 *pp = P->pp[slot].p, *pq = P->pq[slot].p;
     if (nl) launch_project(P, tabs, nb, X, ldx, pp, pq, st);    // projections read the INPUT orbitals
-    const Fft3Args fa = fft3_args(P, nb, X, ldx, HX, ldhx);
-    cudaError_t ke = cudaSuccess;
-    RS_DISPATCH_N(ke, Nz, launch_fwd_zy, fa, P->num_sms, st)              // z fwd, y fwd stage A:  X -> HX
-    RS_CUDA(ke);
-    RS_DISPATCH_N(ke, Nx, launch_x, fa, P->num_sms, st)                   // y B, x fwd, t(k)/Ng, x inv, y B'
-    RS_CUDA(ke);
-    RS_DISPATCH_N(ke, Nz, launch_inv_yz, fa, P->num_sms, st)              // y A', z inv, + v(r) psi(r)
-    RS_CUDA(ke);
-    P->last_launches += 3;
+    for (int c0 = 0; c0 < nb; c0 += fft_batch) {
+        const Fft3Args fa = fft3_args(P, std::min(fft_batch, nb - c0), X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx);
+        cudaError_t ke = cudaSuccess;
+        RS_DISPATCH_N(ke, Nz, launch_fwd_zy, fa, P->num_sms, st)              // z fwd, y fwd stage A:  X -> HX
+        RS_CUDA(ke);
+        RS_DISPATCH_N(ke, Nx, launch_x, fa, P->num_sms, st)                   // y B, x fwd, t(k)/Ng, x inv, y B'
+        RS_CUDA(ke);
+        RS_DISPATCH_N(ke, Nz, launch_inv_yz, fa, P->num_sms, st)              // y A', z inv, + v(r) psi(r)
+        RS_CUDA(ke);
+        P->last_launches += 3;
+    }
     if (nl) launch_scatter(P, tabs, nb, pq, HX, ldhx, st);
     RS_CUDA(cudaGetLastError());
     return RSDFT_OK;
@@ -715,12 +724,16 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
     const int batch = P->user_batch > 0 ? P->user_batch : default_batch(P);
     P->batch = batch;
     if (P->pipeline && pipeline_available(P->n)) return apply_h_pipeline(P, ncol, X, ldx, HX, ldhx, batch, st);
-    const int nbatches = (ncol + batch - 1) / batch;
-    const int ns = std::max(1, std::min(std::min(P->nstreams, (int)rsdft_plan::MAX_STREAMS), nbatches));
+    // With large projector tables (configs 3, 4: 43 / 98 MB of beta) the projector kernels work on units of 4 FFT
+    // batches: project and scatter read beta once per unit, so its traffic per column drops 4x.
+    const bool big_beta = P->natom > 0 && P->beta.bytes() >= ((size_t)32 << 20);
+    const int unit = P->user_batch > 0 ? batch : (big_beta ? std::min(4 * batch, 64) : batch);
+    const int nunits = (ncol + unit - 1) / unit;
+    const int ns = std::max(1, std::min(std::min(P->nstreams, (int)rsdft_plan::MAX_STREAMS), nunits));
     if (P->natom > 0 && P->total_pts > 0)
         for (int i = 0; i < ns; ++i) {
-            RS_CUDA(P->pp[i].ensure((size_t)P->nchunks * P->maxproj * batch));
-            RS_CUDA(P->pq[i].ensure((size_t)P->natom * P->maxproj * batch));
+            RS_CUDA(P->pp[i].ensure((size_t)P->nchunks * P->maxproj * unit));
+            RS_CUDA(P->pq[i].ensure((size_t)P->natom * P->maxproj * unit));
         }
     if (ns > 1) {
         if (!P->ev_fork) RS_CUDA(cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming));
@@ -729,10 +742,10 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
             if (!P->ev_join[i]) RS_CUDA(cudaEventCreateWithFlags(&P->ev_join[i], cudaEventDisableTiming));
         }
     }
-    // With large projector tables (configs 3, 4: 43 / 98 MB of beta) the streams are re-aligned after every
-    // round of ns batches: concurrent project/scatter kernels of the ns streams then read the same beta
-    // lines through L2 (measured +6-8 %); with small tables free-running streams are as fast or faster.
-    const bool rounds = ns > 1 && P->beta.bytes() >= ((size_t)32 << 20);
+    // the streams are re-aligned after every round of ns units: concurrent project/scatter kernels of the ns
+    // streams then read the same beta lines through L2 (measured +6-8 %); with small tables free-running streams
+    // are as fast or faster.
+    const bool rounds = ns > 1 && big_beta;
     auto fork = [&]() -> cudaError_t {      // the internal streams start after everything already queued on `st`
         cudaError_t e = cudaEventRecord(P->ev_fork, st);
         for (int i = 0; i < ns && e == cudaSuccess; ++i) e = cudaStreamWaitEvent(P->s_batch[i], P->ev_fork, 0);
@@ -748,14 +761,14 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
     };
     if (ns > 1) RS_CUDA(fork());
     int k = 0;
-    for (int c0 = 0; c0 < ncol; c0 += batch, ++k) {
-        const int nb = std::min(batch, ncol - c0);
+    for (int c0 = 0; c0 < ncol; c0 += unit, ++k) {
+        const int nb = std::min(unit, ncol - c0);
         const int slot = ns > 1 ? k % ns : 0;
         if (rounds && k > 0 && slot == 0) {
             RS_CUDA(join());
             RS_CUDA(fork());
         }
-        const int rc = apply_h_batch(P, slot, nb, X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx,
+        const int rc = apply_h_batch(P, slot, nb, batch, X + (int64_t)c0 * ldx, ldx, HX + (int64_t)c0 * ldhx, ldhx,
                                      ns > 1 ? P->s_batch[slot] : st);
         if (rc != RSDFT_OK) {
             if (ns > 1) (void)join();            // keep the caller's stream ordered after whatever was queued
@@ -798,7 +811,8 @@ int gram_launch(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const doubl
     GramArgs a;
     a.Y = Y; a.HY = HY; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = ntiles; a.kslabs = ks;
     a.nchunks = nchunks; a.tiles = dtiles; a.work = P->gram_work.p;
-    auto kern = gram_dmma_kernel<2, 4, 6, 3, 16, 3>;
+    // operand staging: TMA bulk copies (gram_bulk, rsdft_plan_set_gram_mode) or per-thread cp.async
+    auto kern = P->gram_bulk ? gram_dmma_kernel<2, 4, 6, 3, 16, 3, true> : gram_dmma_kernel<2, 4, 6, 3, 16, 3, false>;
     // the attribute is per device/context: set it on every launch (cheap), never cache it per thread
     RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
     kern<<<ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);
@@ -993,6 +1007,13 @@ int rsdft_plan_set_gram_mode(rsdft_plan_t *plan, int32_t h_upper_only)
     if (!plan || (h_upper_only != 0 && h_upper_only != 1))
         return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_gram_mode: mode must be 0 or 1");
     plan->gram_h_upper = h_upper_only;
+    return RSDFT_OK;
+}
+
+int rsdft_plan_set_gram_staging(rsdft_plan_t *plan, int32_t bulk)
+{
+    if (!plan || (bulk != 0 && bulk != 1)) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_gram_staging: bulk must be 0 or 1");
+    plan->gram_bulk = bulk;
     return RSDFT_OK;
 }
 

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "librsdft.so")
 
 SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram", "rsdft_subspace_rotate",
            "rsdft_subspace_rotate2", "rsdft_subspace_eig", "rsdft_subspace_eig_get", "rsdft_plan_set_eig_mode",
-           "rsdft_subspace_eig_stats", "rsdft_plan_release_workspace", "rsdft_plan_set_pipeline",
+           "rsdft_subspace_eig_stats", "rsdft_plan_release_workspace", "rsdft_plan_set_pipeline", "rsdft_plan_set_gram_staging",
            "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_set_streams", "rsdft_plan_set_gram_mode", "rsdft_plan_destroy",
            "rsdft_last_error"]
 
@@ -83,6 +83,7 @@ def load():
     lib.rsdft_subspace_eig_stats.argtypes = [vp, C.POINTER(C.c_double)]
     lib.rsdft_plan_release_workspace.argtypes = [vp]
     lib.rsdft_plan_set_pipeline.argtypes = [vp, i32]
+    lib.rsdft_plan_set_gram_staging.argtypes = [vp, i32]
     lib.rsdft_block_step_host.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32]
     lib.rsdft_plan_info.argtypes = [vp, C.POINTER(i64)]
     lib.rsdft_plan_set_batch.argtypes = [vp, i32]
@@ -421,6 +422,10 @@ def rsdft_plan_set_streams(plan, nstreams):
 
 def rsdft_plan_set_pipeline(plan, mode):
     _check(load().rsdft_plan_set_pipeline(plan.handle, int(mode)))
+
+
+def rsdft_plan_set_gram_staging(plan, bulk):
+    _check(load().rsdft_plan_set_gram_staging(plan.handle, int(bulk)))
 
 
 def rsdft_plan_set_gram_mode(plan, h_upper_only):

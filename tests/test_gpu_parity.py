@@ -227,6 +227,55 @@ def test_gram_ragged_sizes_and_options(env, n):
     assert torch.equal(torch.view_as_real(H2), torch.view_as_real(H))
 
 
+def test_gram_bulk_copy_staging_is_bitwise_identical(env):
+    """rsdft_plan_set_gram_staging(1): the TMA bulk-copy (cp.async.bulk + mbarrier) operand pipeline computes exactly what
+    the cp.async pipeline computes, ragged last tile and H-upper mode included."""
+    torch, rsdft, wl = env["torch"], env["rsdft"], env["wl"]
+    plan = rsdft.rsdft_plan_create((16, 32, 48), (5.0, 9.0, 14.0))
+    ng = 16 * 32 * 48
+    for n in (7, 200):
+        Y = wl.orbital_block(ng, range(n), 23, 0, device="cuda", ld=ng + 8)
+        HY = wl.orbital_block(ng, range(n), 23, 1, device="cuda")
+        for mode in (0, 1):
+            rsdft.rsdft_plan_set_gram_mode(plan, mode)
+            rsdft.rsdft_plan_set_gram_staging(plan, 0)
+            H0, S0 = rsdft.rsdft_subspace_gram(plan, Y, HY)
+            rsdft.rsdft_plan_set_gram_staging(plan, 1)
+            H1, S1 = rsdft.rsdft_subspace_gram(plan, Y, HY)
+            torch.cuda.synchronize()
+            assert torch.equal(torch.view_as_real(H0), torch.view_as_real(H1))
+            assert torch.equal(torch.view_as_real(S0), torch.view_as_real(S1))
+    plan.close()
+
+
+def test_repeated_calls_are_bitwise_reproducible(env):
+    """Race evidence without a sanitizer (compute-sanitizer is closed on this GPU pool): five repetitions of apply_h with
+    overlapping spheres (colour-class scatter), of the Gram, of the eigen-solve and of rotate2 give identical bits, on
+    both apply_h FFT paths."""
+    torch, rsdft, wl = env["torch"], env["rsdft"], env["wl"]
+    system = wl.small_system(n=(48, 48, 48), L=(9.0, 9.0, 9.0), natom=10, seed=77, nproj=9, rc=2.2)
+    ng = 48 ** 3
+    plan = rsdft.plan_from_system(system)
+    assert rsdft.rsdft_plan_info(plan)["colour_classes"] >= 2
+    Y = wl.orbital_block(ng, range(60), 19, 0, device="cuda")
+    ref = None
+    for rep in range(5):
+        rsdft.rsdft_plan_set_pipeline(plan, rep % 2)
+        HY = torch.full_like(Y, float("nan"))
+        rsdft.rsdft_apply_h(plan, Y, HY)
+        H, S = rsdft.rsdft_subspace_gram(plan, Y, HY)
+        lam, Cm = rsdft.rsdft_subspace_eig(plan, H, S, 20)
+        Xn, HXn, R = rsdft.rsdft_subspace_rotate2(plan, Y, HY, Cm, lam)
+        torch.cuda.synchronize()
+        cur = [torch.view_as_real(t).clone() for t in (HY, H, S, Cm, Xn, HXn, R)] + [lam.clone()]
+        if ref is None:
+            ref = cur
+        else:
+            for a, b in zip(ref, cur):
+                assert torch.equal(a, b)
+    plan.close()
+
+
 def test_gram_plane_waves_closed_form(env):
     """Plane-wave columns: S_sub = Ng I, H_sub = Ng diag(t) (V = 0, no projectors) -- closed form."""
     torch, rsdft = env["torch"], env["rsdft"]
