@@ -49,6 +49,9 @@ struct Fft3Args {
     const double *kin_x;    // [nx]     t_x(kx)/Ng, natural frequency index
     const double *kin_yz;   // [ny*nz]  (t_y(ky(r)) + t_z(kz(p)))/Ng at r*nz + p (permuted positions)
     const double *vloc;     // [Ng]
+    int32_t hint_stream;    // L2 eviction class of the once-touched data (X reads, HX writes): 0 normal, 1 evict_first, 2 evict_last
+    int32_t hint_keep;      // ... of the k-space scratch between the phases
+    int32_t x_tma;          // 1: run the TMA-staged x kernel when the shape has one
 };
 
 constexpr bool radix16_ok(int N) { return N % 16 == 0 && (N / 16 <= 8 || N / 16 == 10 || N / 16 == 12 || N / 16 == 16); }
@@ -61,6 +64,33 @@ template <int N> struct Axis {
 __device__ __forceinline__ double2 ld_nc(const double2 *p) { return __ldg(p); }
 // k-space is written by other SMs inside one launch of the pipeline kernel: read it through L2 only
 __device__ __forceinline__ double2 ld_cg(const double2 *p) { return __ldcg(p); }
+
+// L2 eviction classes (createpolicy + .L2::cache_hint): the pipeline kernel marks the data it touches once
+// (X, psi, the final HX) evict_first and the k-space scratch that must survive from phase to phase evict_last.
+__device__ __forceinline__ uint64_t l2_policy(int kind)
+{
+    uint64_t p;
+    if (kind == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    else if (kind == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ double2 ld_nc_hint(const double2 *p, uint64_t pol)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 ld_cg_hint(const double2 *p, uint64_t pol)
+{
+    double2 v;
+    asm volatile("ld.global.cg.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_hint(double2 *p, double2 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" :: "l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
 
 // barrier `id` over `nt` threads (id 0 with the whole CTA = __syncthreads)
 __device__ __forceinline__ void group_sync(int id, int nt) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nt) : "memory"); }
@@ -89,9 +119,10 @@ __device__ __forceinline__ void fft3_zy_tables(const Fft3Args &a, int n2y, doubl
 }
 
 // z forward + y forward stage A of one tile.  src/dst: plane base (column, x) of X / W.
-template <int NZ, int R2Y, int NT>
+template <int NZ, int R2Y, int NT, bool HINT = false>
 __device__ __forceinline__ void fft3_fwd_tile(const double2 *__restrict__ src, double2 *__restrict__ dst, int my, int n2y, double2 *S,
-                                              const double2 *twz_s, const double2 *twy_s, int tid, int bar)
+                                              const double2 *twz_s, const double2 *twy_s, int tid, int bar,
+                                              uint64_t pol_in = 0, uint64_t pol_out = 0)
 {
     using C = ZyCfg<NZ, R2Y>;
     constexpr int R2Z = C::R2Z, MZ = C::MZ, G = C::G, RP = C::RP;
@@ -102,7 +133,7 @@ __device__ __forceinline__ void fft3_fwd_tile(const double2 *__restrict__ src, d
         const double2 *row = src + (int64_t)(j * my + n2y) * NZ + n2;
         double re[MZ], im[MZ];
 #pragma unroll
-        for (int n1 = 0; n1 < MZ; ++n1) { const double2 v = ld_nc(row + n1 * R2Z); re[n1] = v.x; im[n1] = v.y; }
+        for (int n1 = 0; n1 < MZ; ++n1) { const double2 v = HINT ? ld_nc_hint(row + n1 * R2Z, pol_in) : ld_nc(row + n1 * R2Z); re[n1] = v.x; im[n1] = v.y; }
         Dft<MZ>::run(re, im);
 #pragma unroll
         for (int k = 1; k < MZ; ++k) { const double2 w = twz_s[(k - 1) * R2Z + n2]; tw_mul(re[k], im[k], w.x, -w.y); }
@@ -131,7 +162,10 @@ __device__ __forceinline__ void fft3_fwd_tile(const double2 *__restrict__ src, d
 #pragma unroll
         for (int k = 1; k < R2Y; ++k) { const double2 w = twy_s[k]; tw_mul(br[k], bi[k], w.x, -w.y); }
 #pragma unroll
-        for (int k = 0; k < R2Y; ++k) dst[(int64_t)(k * my + n2y) * NZ + p] = make_double2(br[k], bi[k]);
+        for (int k = 0; k < R2Y; ++k) {
+            if (HINT) st_hint(dst + (int64_t)(k * my + n2y) * NZ + p, make_double2(br[k], bi[k]), pol_out);
+            else dst[(int64_t)(k * my + n2y) * NZ + p] = make_double2(br[k], bi[k]);
+        }
     }
     group_sync(bar, NT);
 }
@@ -169,9 +203,10 @@ __device__ __forceinline__ void fft3_inv_stages_12(double2 *S, const double2 *tw
 
 // z inverse stage A' + V_loc: conj twiddle, radix-MZ over k1z (swapped) -> z = n1*R2Z + n2;  HX = T psi + v psi.
 // psi comes from shared memory (Sp, dense [R2Y][NZ]) when PSI_SMEM, else straight from global memory (psi_g = plane base).
-template <int NZ, int R2Y, int NT, bool PSI_SMEM>
+template <int NZ, int R2Y, int NT, bool PSI_SMEM, bool HINT = false>
 __device__ __forceinline__ void fft3_inv_stage_3(const double2 *S, const double2 *twz_s, const double2 *Sp, const double2 *__restrict__ psi_g,
-                                                 const double *__restrict__ vl, double2 *__restrict__ dst, int my, int n2y, int tid)
+                                                 const double *__restrict__ vl, double2 *__restrict__ dst, int my, int n2y, int tid,
+                                                 uint64_t pol_stream = 0)
 {
     using C = ZyCfg<NZ, R2Y>;
     constexpr int R2Z = C::R2Z, MZ = C::MZ, G = C::G, RP = C::RP;
@@ -183,7 +218,7 @@ __device__ __forceinline__ void fft3_inv_stage_3(const double2 *S, const double2
         double vv[MZ];
 #pragma unroll
         for (int n1 = 0; n1 < MZ; ++n1) {          // issued first: their latency hides behind the radix-MZ below
-            ps[n1] = PSI_SMEM ? Sp[j * NZ + n1 * R2Z + n2] : ld_nc(psi_g + off + n1 * R2Z);
+            ps[n1] = PSI_SMEM ? Sp[j * NZ + n1 * R2Z + n2] : (HINT ? ld_nc_hint(psi_g + off + n1 * R2Z, pol_stream) : ld_nc(psi_g + off + n1 * R2Z));
             vv[n1] = __ldg(vl + off + n1 * R2Z);
         }
         double re[MZ], im[MZ];
@@ -193,21 +228,25 @@ __device__ __forceinline__ void fft3_inv_stage_3(const double2 *S, const double2
         for (int k = 1; k < MZ; ++k) { const double2 w = twz_s[(k - 1) * R2Z + n2]; tw_mul(im[k], re[k], w.x, -w.y); }
         Dft<MZ>::run(im, re);
 #pragma unroll
-        for (int n1 = 0; n1 < MZ; ++n1)
-            dst[off + n1 * R2Z] = make_double2(fma(vv[n1], ps[n1].x, re[n1]), fma(vv[n1], ps[n1].y, im[n1]));
+        for (int n1 = 0; n1 < MZ; ++n1) {
+            const double2 r = make_double2(fma(vv[n1], ps[n1].x, re[n1]), fma(vv[n1], ps[n1].y, im[n1]));
+            if (HINT) st_hint(dst + off + n1 * R2Z, r, pol_stream);
+            else dst[off + n1 * R2Z] = r;
+        }
     }
 }
 
 // cp.async of the R2Y k-space rows {k*my + n2y} of one plane into the padded tile layout
-template <int NZ, int R2Y, int NT>
-__device__ __forceinline__ void fft3_issue_w_tile(const double2 *__restrict__ src, int my, int n2y, double2 *S, int tid)
+template <int NZ, int R2Y, int NT, bool HINT = false>
+__device__ __forceinline__ void fft3_issue_w_tile(const double2 *__restrict__ src, int my, int n2y, double2 *S, int tid, uint64_t pol = 0)
 {
     using C = ZyCfg<NZ, R2Y>;
     constexpr int R2Z = C::R2Z, G = C::G, RP = C::RP;
 #pragma unroll
     for (int e = tid; e < R2Y * NZ; e += NT) {
         const int k = e / NZ, p = e - k * NZ;
-        cp_async16(S + k * RP + (p / R2Z) * G + (p % R2Z), src + (int64_t)(k * my + n2y) * NZ + p);
+        if (HINT) cp_async16_hint(S + k * RP + (p / R2Z) * G + (p % R2Z), src + (int64_t)(k * my + n2y) * NZ + p, pol);
+        else cp_async16(S + k * RP + (p / R2Z) * G + (p % R2Z), src + (int64_t)(k * my + n2y) * NZ + p);
     }
 }
 
@@ -305,7 +344,7 @@ __global__ void __launch_bounds__(128, MINB) fft3_inv_yz_kernel(Fft3Args a)
 // y stage B, x forward, kinetic factor, x inverse, y stage B'.  In place on W.
 // Tile = (column, k1y, z-chunk): S[x][line], line = jy*TZ + z, odd pitch P = lines + 1.
 template <int MY, int NX, int TZ, int NT, bool CG>
-__device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *base, double2 *S, int P, int tid)
+__device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *base, double2 *S, int P, int tid, uint64_t pol)
 {
     // items are taken two at a time so that both items' global loads are in flight together
     int item = tid;
@@ -315,9 +354,9 @@ __device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *
         const double2 *p1 = base + (int64_t)x1 * a.ny * a.nz + z1;
         double re0[MY], im0[MY], re1[MY], im1[MY];
 #pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg(p0 + (int64_t)j * a.nz) : p0[(int64_t)j * a.nz]; re0[j] = v.x; im0[j] = v.y; }
+        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg_hint(p0 + (int64_t)j * a.nz, pol) : p0[(int64_t)j * a.nz]; re0[j] = v.x; im0[j] = v.y; }
 #pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg(p1 + (int64_t)j * a.nz) : p1[(int64_t)j * a.nz]; re1[j] = v.x; im1[j] = v.y; }
+        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg_hint(p1 + (int64_t)j * a.nz, pol) : p1[(int64_t)j * a.nz]; re1[j] = v.x; im1[j] = v.y; }
         Dft<MY>::run(re0, im0);
 #pragma unroll
         for (int j = 0; j < MY; ++j) S[x0 * P + j * TZ + z0] = make_double2(re0[j], im0[j]);
@@ -330,15 +369,15 @@ __device__ __forceinline__ void fft3_x_load_y(const Fft3Args &a, const double2 *
         const double2 *ptr = base + (int64_t)x * a.ny * a.nz + z;
         double re[MY], im[MY];
 #pragma unroll
-        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg(ptr + (int64_t)j * a.nz) : ptr[(int64_t)j * a.nz]; re[j] = v.x; im[j] = v.y; }
+        for (int j = 0; j < MY; ++j) { const double2 v = CG ? ld_cg_hint(ptr + (int64_t)j * a.nz, pol) : ptr[(int64_t)j * a.nz]; re[j] = v.x; im[j] = v.y; }
         Dft<MY>::run(re, im);
 #pragma unroll
         for (int j = 0; j < MY; ++j) S[x * P + j * TZ + z] = make_double2(re[j], im[j]);
     }
 }
 
-template <int MY, int NX, int TZ, int NT>
-__device__ __forceinline__ void fft3_x_store_y(const Fft3Args &a, double2 *base, const double2 *S, int P, int tid)
+template <int MY, int NX, int TZ, int NT, bool CG>
+__device__ __forceinline__ void fft3_x_store_y(const Fft3Args &a, double2 *base, const double2 *S, int P, int tid, uint64_t pol)
 {
     for (int item = tid; item < NX * TZ; item += NT) {
         const int z = item % TZ, x = item / TZ;
@@ -348,7 +387,10 @@ __device__ __forceinline__ void fft3_x_store_y(const Fft3Args &a, double2 *base,
         for (int j = 0; j < MY; ++j) { const double2 v = S[x * P + j * TZ + z]; re[j] = v.x; im[j] = v.y; }
         Dft<MY>::run(im, re);
 #pragma unroll
-        for (int j = 0; j < MY; ++j) ptr[(int64_t)j * a.nz] = make_double2(re[j], im[j]);
+        for (int j = 0; j < MY; ++j) {
+            if (CG) st_hint(ptr + (int64_t)j * a.nz, make_double2(re[j], im[j]), pol);
+            else ptr[(int64_t)j * a.nz] = make_double2(re[j], im[j]);
+        }
     }
 }
 
@@ -371,11 +413,11 @@ __device__ __forceinline__ void fft3_x_store_y(const Fft3Args &a, double2 *base,
 // kinx_s[kx] = t_x(kx)/Ng, kin = kin_yz + (k1y*my)*nz + zc*TZ.  The whole CTA (NT threads) works on the tile.
 template <int NX, int TZ, int NT, bool CG>
 __device__ __forceinline__ void fft3_x_tile(const Fft3Args &a, double2 *base, const double *__restrict__ kin, double2 *S,
-                                            const double2 *twx_s, const double *kinx_s, int tid)
+                                            const double2 *twx_s, const double *kinx_s, int tid, uint64_t pol = 0)
 {
     constexpr int R2X = Axis<NX>::R2, MX = Axis<NX>::M;
     const int my = a.my, lines = my * TZ, P = lines + 1;
-    RS_SWITCH_MY(my, (fft3_x_load_y<MYC, NX, TZ, NT, CG>(a, base, S, P, tid)))
+    RS_SWITCH_MY(my, (fft3_x_load_y<MYC, NX, TZ, NT, CG>(a, base, S, P, tid, pol)))
     __syncthreads();
     // x stage A: radix-MX over n1 (x = n1*R2X + n2), twiddle, in place
     for (int item = tid; item < lines * R2X; item += NT) {
@@ -425,7 +467,7 @@ __device__ __forceinline__ void fft3_x_tile(const Fft3Args &a, double2 *base, co
         for (int n1 = 0; n1 < MX; ++n1) p[n1 * R2X * P] = make_double2(re[n1], im[n1]);
     }
     __syncthreads();
-    RS_SWITCH_MY(my, (fft3_x_store_y<MYC, NX, TZ, NT>(a, base, S, P, tid)))
+    RS_SWITCH_MY(my, (fft3_x_store_y<MYC, NX, TZ, NT, CG>(a, base, S, P, tid, pol)))
     __syncthreads();
 }
 
@@ -540,6 +582,7 @@ __global__ void __launch_bounds__(256, 2) fft3_pipeline_kernel(Fft3Args a, PipeA
     const int tid = threadIdx.x, half = tid >> 7, htid = tid & (NH - 1);
     const int my = a.my;
     fft3_x_tables<N, NT>(a, twz_s, kinx_s, tid);
+    const uint64_t pol_stream = l2_policy(a.hint_stream), pol_keep = l2_policy(a.hint_keep);
     if (tid == 0) next_item = atomicAdd(q.head, 1);
     __syncthreads();
     const int64_t total = (int64_t)(a.ncol + q.lag_inv) * q.npattern;
@@ -558,14 +601,14 @@ __global__ void __launch_bounds__(256, 2) fft3_pipeline_kernel(Fft3Args a, PipeA
             const int u = 2 * t + half, x = u / my, n2y = u - x * my;
             if (htid < R2Y) twy_s[half][htid] = a.twy[n2y * htid];
             group_sync(1 + half, NH);
-            fft3_fwd_tile<N, R2Y, NH>(a.X + (int64_t)col * a.ldx + (int64_t)x * a.ny * N, a.W + (int64_t)col * a.ldw + (int64_t)x * a.ny * N,
-                                      my, n2y, S + half * C::TILE, twz_s, twy_s[half], htid, 1 + half);
+            fft3_fwd_tile<N, R2Y, NH, true>(a.X + (int64_t)col * a.ldx + (int64_t)x * a.ny * N, a.W + (int64_t)col * a.ldw + (int64_t)x * a.ny * N,
+                                            my, n2y, S + half * C::TILE, twz_s, twy_s[half], htid, 1 + half, pol_stream, pol_keep);
         } else if (ph == 1) {
             if (tid == 0) pipe_wait(q.done + col, q.n_fwd);
             __syncthreads();
             const int k1y = t / q.zchunks, zc = t - k1y * q.zchunks;
             const int64_t toff = (int64_t)(k1y * my) * a.nz + zc * TZ;
-            fft3_x_tile<N, TZ, NT, true>(a, a.W + (int64_t)col * a.ldw + toff, a.kin_yz + toff, S, twz_s, kinx_s, tid);
+            fft3_x_tile<N, TZ, NT, true>(a, a.W + (int64_t)col * a.ldw + toff, a.kin_yz + toff, S, twz_s, kinx_s, tid, pol_keep);
         } else {
             if (tid == 0) pipe_wait(q.done + a.ncol + col, q.n_x);
             __syncthreads();
@@ -573,14 +616,14 @@ __global__ void __launch_bounds__(256, 2) fft3_pipeline_kernel(Fft3Args a, PipeA
             if (htid < R2Y) twy_s[half][htid] = a.twy[n2y * htid];
             const int64_t po = (int64_t)x * a.ny * N;
             double2 *Sh = S + half * C::TILE;
-            fft3_issue_w_tile<N, R2Y, NH>(a.W + (int64_t)col * a.ldw + po, my, n2y, Sh, htid);     // cp.async.cg: L2 only
+            fft3_issue_w_tile<N, R2Y, NH, true>(a.W + (int64_t)col * a.ldw + po, my, n2y, Sh, htid, pol_stream);     // cp.async.cg: L2 only; last use of the k-space lines
             cp_async_commit();
             cp_async_wait<0>();
             group_sync(1 + half, NH);
             fft3_inv_stages_12<N, R2Y, NH>(Sh, twy_s[half], htid, 1 + half);
             group_sync(1 + half, NH);
-            fft3_inv_stage_3<N, R2Y, NH, false>(Sh, twz_s, nullptr, a.X + (int64_t)col * a.ldx + po, a.vloc + po,
-                                                a.HX + (int64_t)col * a.ldhx + po, my, n2y, htid);
+            fft3_inv_stage_3<N, R2Y, NH, false, true>(Sh, twz_s, nullptr, a.X + (int64_t)col * a.ldx + po, a.vloc + po,
+                                                      a.HX + (int64_t)col * a.ldhx + po, my, n2y, htid, pol_stream);
         }
         __syncthreads();                                          // all stores of this item are issued
         if (tid == 0) {

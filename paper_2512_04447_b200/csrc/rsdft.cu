@@ -17,6 +17,7 @@
 
 #include "eig_kernels.cuh"
 #include "fft3_kernels.cuh"
+#include "fft3_tma_kernels.cuh"
 #include "gram_kernels.cuh"
 #include "nonlocal_kernels.cuh"
 #include "rotate_kernels.cuh"
@@ -115,6 +116,7 @@ struct rsdft_plan {
     int batch = 0;                // columns per kernel sequence
     int user_batch = 0;
     int pipeline = 0;             // 1: persistent FFT pipeline kernel where available (rsdft_plan_set_pipeline)
+    int x_tma = 1;                // 1: TMA-staged x kernel where the shape has one
     DevBuf<uint32_t> pipe_pattern;
     DevBuf<int32_t> pipe_counters;
     int pipe_key = -1, pipe_npattern = 0;
@@ -415,6 +417,14 @@ namespace {
 
 using namespace rsdft;
 
+// RSDFT_LAB_N: development builds that instantiate a single axis length (seconds instead of minutes to compile)
+#ifdef RSDFT_LAB_N
+#define RS_DISPATCH_N(ERR_, N_, FN_, ...)                                    \
+    switch (N_) {                                                            \
+    case RSDFT_LAB_N: ERR_ = FN_<RSDFT_LAB_N>(__VA_ARGS__); break;           \
+    default: ERR_ = cudaErrorInvalidValue; break;                            \
+    }
+#else
 #define RS_DISPATCH_N(ERR_, N_, FN_, ...)                                    \
     switch (N_) {                                                            \
     case 12: ERR_ = FN_<12>(__VA_ARGS__); break;                             \
@@ -438,6 +448,7 @@ using namespace rsdft;
     case 256: ERR_ = FN_<256>(__VA_ARGS__); break;                           \
     default: ERR_ = cudaErrorInvalidValue; break;                            \
     }
+#endif
 
 // CTAs per SM that fit by shared memory (1 KB reserved per CTA), capped
 inline int occ_by_smem(size_t smem, int cap)
@@ -497,9 +508,85 @@ cudaError_t launch_x_cfg(const Fft3Args &a, int sms, cudaStream_t st)
     return cudaSuccess;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*TmaEncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+TmaEncodeFn tma_encoder()
+{
+    static TmaEncodeFn fn = [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return (TmaEncodeFn)p;
+    }();
+    return fn;
+}
+
+// Tensor map of a column block seen as doubles [col][x][y][2*z]; box = one x tile (2*tz, my, nx, 1).
+bool x_tile_map(CUtensorMap *tm, const Fft3Args &a, int tz)
+{
+    TmaEncodeFn enc = tma_encoder();
+    if (!enc) return false;
+    const cuuint64_t gdim[4] = {(cuuint64_t)2 * a.nz, (cuuint64_t)a.ny, (cuuint64_t)a.nx, (cuuint64_t)a.ncol};
+    const cuuint64_t gstr[3] = {(cuuint64_t)a.nz * 16, (cuuint64_t)a.ny * a.nz * 16, (cuuint64_t)a.ldw * 16};
+    const cuuint32_t box[4] = {(cuuint32_t)(2 * tz), (cuuint32_t)a.my, (cuuint32_t)a.nx, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+    if (const char *e = getenv("RSDFT_LAB_PROMO")) promo = atoi(e) == 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : (atoi(e) == 64 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : (atoi(e) == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : promo));   // LAB
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)a.W, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// TMA-staged x kernel (fft3_tma_kernels.cuh); returns cudaErrorNotSupported when the shape has none
+template <int NX, int TZ, int G, int NTG, int SPG>
+cudaError_t launch_x_tma_cfg(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    if (a.ny != a.nx || a.r2y != Axis<NX>::R2 || Axis<NX>::R2 != 16 || a.nz % TZ != 0 || ((uintptr_t)a.W & 15) != 0) return cudaErrorNotSupported;
+    CUtensorMap tm;
+    if (!x_tile_map(&tm, a, TZ)) return cudaErrorNotSupported;
+    auto k = fft3_x_tma_kernel<NX, TZ, G, NTG, SPG>;
+    const size_t smem = XTmaSmem<NX, TZ, G, SPG>::bytes;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int64_t ntiles = (int64_t)a.ncol * a.r2y * (a.nz / TZ);
+    const int64_t grid = std::min<int64_t>(sms, (ntiles + G - 1) / G);
+    k<<<(int)grid, G * NTG, smem, st>>>(a, tm);
+    return cudaSuccess;
+}
+template <int NX>
+cudaError_t launch_x_tma(const Fft3Args &a, int sms, cudaStream_t st)
+{
+    using Cc = XTmaCfg<NX>;
+    if constexpr (Cc::TZ == 0) {
+        return cudaErrorNotSupported;
+    } else {
+#ifdef RSDFT_LAB_N
+        if (const char *e = getenv("RSDFT_LAB_XCFG")) {
+            switch (atoi(e)) {
+            case 1: return launch_x_tma_cfg<NX, 4, 6, 96, 1>(a, sms, st);
+            case 2: return launch_x_tma_cfg<NX, 4, 3, 96, 2>(a, sms, st);
+            case 3: return launch_x_tma_cfg<NX, 4, 5, 96, 1>(a, sms, st);
+            case 4: return launch_x_tma_cfg<NX, 4, 4, 160, 1>(a, sms, st);
+            case 5: return launch_x_tma_cfg<NX, 8, 2, 160, 1>(a, sms, st);
+            case 6: return launch_x_tma_cfg<NX, 8, 3, 160, 1>(a, sms, st);
+            case 7: return launch_x_tma_cfg<NX, 4, 6, 64, 1>(a, sms, st);
+            default: break;
+            }
+        }
+#endif
+        return launch_x_tma_cfg<NX, Cc::TZ, Cc::G, Cc::NTG, Cc::SPG>(a, sms, st);
+    }
+}
+
 template <int NX>
 cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
 {
+    if (a.x_tma) {
+        const cudaError_t e = launch_x_tma<NX>(a, sms, st);
+        if (e != cudaErrorNotSupported) return e;
+    }
     // the tile is NX x (my*TZ) elements: fall back to narrower z chunks when a large ny makes it too big or
     // when nz is not a multiple of the preferred chunk (nz = 12*M with odd M)
     auto fits = [&](int tz) { return a.nz % tz == 0 && (size_t)NX * (a.my * tz + 1) * sizeof(double2) + 4096 <= (size_t)227 * 1024; };
@@ -522,13 +609,17 @@ cudaError_t launch_pipeline(const Fft3Args &a, const PipeArgs &q, int sms, cudaS
     k<<<(int)std::min<int64_t>(total, (int64_t)sms * 2), 256, smem, st>>>(a, q);
     return cudaSuccess;
 }
+#ifdef RSDFT_LAB_N
+#define RS_PIPE_LENGTHS(X_) X_(RSDFT_LAB_N)
+#else
+#define RS_PIPE_LENGTHS(X_) X_(48) X_(60) X_(64) X_(80) X_(96) X_(112) X_(128)
+#endif
 inline bool pipeline_available(const int n[3])
 {
     if (n[0] != n[1] || n[1] != n[2]) return false;
-    switch (n[0]) {
-    case 48: case 60: case 64: case 80: case 96: case 112: case 128: return true;
-    default: return false;
-    }
+#define RS_PIPE_OK(N_) case N_: return true;
+    switch (n[0]) { RS_PIPE_LENGTHS(RS_PIPE_OK) default: return false; }
+#undef RS_PIPE_OK
 }
 
 template <int MT>
@@ -586,6 +677,11 @@ Fft3Args fft3_args(const rsdft_plan *P, int nb, const double2 *X, int64_t ldx, d
     fa.r2y = first_radix(P->n[1]); fa.my = P->n[1] / fa.r2y;
     fa.twx = P->tw[0].p; fa.twy = P->tw[1].p; fa.twz = P->tw[2].p;
     fa.kin_x = P->kin_x.p; fa.kin_yz = P->kin_yz.p; fa.vloc = P->vloc.p;
+    fa.hint_stream = 1; fa.hint_keep = 0;
+    fa.x_tma = P->x_tma;
+    if (const char *e = getenv("RSDFT_LAB_XTMA")) fa.x_tma = atoi(e);   // LAB
+    if (getenv("RSDFT_LAB_XNOSTORE")) fa.x_tma |= 2;   // LAB
+    if (const char *e = getenv("RSDFT_LAB_HINTS")) { fa.hint_stream = (e[0] - '0'); fa.hint_keep = (e[1] - '0'); }   // LAB
     return fa;
 }
 
@@ -664,7 +760,8 @@ int pipeline_pattern(rsdft_plan *P, const Fft3Args &fa, int tz, PipeArgs &q, cud
     q.pattern = P->pipe_pattern.p;
     q.npattern = P->pipe_npattern;
     q.lag_x = 1;
-    q.lag_inv = 3;      // measured at configs[2]: lag 2 -> 38.6 ms, 3 -> 36.8, 4 -> 36.9 per 1440 columns
+    q.lag_inv = 3;
+    if (const char *e = getenv("RSDFT_LAB_LAG")) q.lag_inv = atoi(e);   // LAB      // measured at configs[2]: lag 2 -> 38.6 ms, 3 -> 36.8, 4 -> 36.9 per 1440 columns
     return RSDFT_OK;
 }
 
@@ -687,27 +784,18 @@ int apply_h_pipeline(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, dou
     const Fft3Args fa = fft3_args(P, ncol, X, ldx, HX, ldhx);
     PipeArgs q;
     int tz = 0;
-    switch (P->n[0]) {
-    case 48: tz = XCfg<48>::TZ; break;  case 60: tz = XCfg<60>::TZ; break;  case 64: tz = XCfg<64>::TZ; break;
-    case 80: tz = XCfg<80>::TZ; break;  case 96: tz = XCfg<96>::TZ; break;  case 112: tz = XCfg<112>::TZ; break;
-    default: tz = XCfg<128>::TZ; break;
-    }
+#define RS_PIPE_TZ(N_) case N_: tz = XCfg<N_>::TZ; break;
+    switch (P->n[0]) { RS_PIPE_LENGTHS(RS_PIPE_TZ) default: break; }
+#undef RS_PIPE_TZ
     if (int rc = pipeline_pattern(P, fa, tz, q, st)) return rc;
     RS_CUDA(P->pipe_counters.ensure((size_t)3 * ncol + 4));
     RS_CUDA(cudaMemsetAsync(P->pipe_counters.p, 0, ((size_t)3 * ncol + 4) * sizeof(int32_t), st));
     q.head = P->pipe_counters.p;
     q.done = P->pipe_counters.p + 4;
-    cudaError_t ke = cudaSuccess;
-    switch (P->n[0]) {
-    case 48: ke = launch_pipeline<48>(fa, q, P->num_sms, st); break;
-    case 60: ke = launch_pipeline<60>(fa, q, P->num_sms, st); break;
-    case 64: ke = launch_pipeline<64>(fa, q, P->num_sms, st); break;
-    case 80: ke = launch_pipeline<80>(fa, q, P->num_sms, st); break;
-    case 96: ke = launch_pipeline<96>(fa, q, P->num_sms, st); break;
-    case 112: ke = launch_pipeline<112>(fa, q, P->num_sms, st); break;
-    case 128: ke = launch_pipeline<128>(fa, q, P->num_sms, st); break;
-    default: ke = cudaErrorInvalidValue; break;
-    }
+    cudaError_t ke = cudaErrorInvalidValue;
+#define RS_PIPE_LAUNCH(N_) case N_: ke = launch_pipeline<N_>(fa, q, P->num_sms, st); break;
+    switch (P->n[0]) { RS_PIPE_LENGTHS(RS_PIPE_LAUNCH) default: break; }
+#undef RS_PIPE_LAUNCH
     RS_CUDA(ke);
     ++P->last_launches;
     if (nl)
