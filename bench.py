@@ -57,7 +57,7 @@ def parse():
     ap.add_argument("--batch", type=int, default=0, help="apply_h column batch width (0 = library default)")
     ap.add_argument("--streams", type=int, default=0, help="apply_h internal streams (0 = library default)")
     ap.add_argument("--ncol-per-call", type=int, default=0, help="columns per rsdft_apply_h call (config 4 sweep)")
-    ap.add_argument("--pipeline", type=int, default=-1, help="apply_h FFT path: 0 three kernels per batch, 1 persistent pipeline kernel (-1 = library default)")
+    ap.add_argument("--pipeline", type=int, default=-1, help="apply_h FFT path: 0 three kernels per batch, 1 persistent pipeline kernel, 2 three kernels with the TMA x kernel (-1 = library default)")
     return ap.parse_args()
 
 
@@ -466,6 +466,16 @@ def run_ours(args):
     t_apply, t_gram = st["t_apply"], st["t_gram"]
     clocks = row["clocks"]
 
+    # ---- the three FFT paths of rsdft_apply_h on the same block (informational; the headline ran the library default)
+    paths = {}
+    for mode, name in ((0, "three_kernels"), (1, "pipeline_kernel"), (2, "three_kernels_tma_x")):
+        rsdft.rsdft_plan_set_pipeline(plan, mode)
+        paths[name + "_ms"] = 1e3 * timed(torch, lambda: rsdft.rsdft_apply_h(plan, Y, HY), 2)
+    rsdft.rsdft_plan_set_pipeline(plan, args.pipeline if args.pipeline >= 0 else 3)
+    paths["note"] = ("rsdft_plan_set_pipeline 0 / 1 / 2 on the headline block, ms per apply_h call; bitwise identical results (tests); "
+                     "the pipeline kernel keeps k-space in L2 (58 B of DRAM traffic per orbital*point against 112) but is bound by the "
+                     "SM's L1/shared-memory data pipe, see DESIGN.md")
+
     # ---- optional Gram mode (H_sub from its upper tiles, mirrored): informational, not the headline
     rsdft.rsdft_plan_set_gram_mode(plan, 1)
     Hs2 = torch.empty_like(Hs)
@@ -641,7 +651,7 @@ def run_ours(args):
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64 (complex128)",
                 data="synthetic", config=dict(workload=workload_name(args.config), l2="inputs %.1f GB per block >> 126 MB L2, no flush needed" % (n * ng * 16 / 1e9),
                                               ncol_per_apply_call=row["ncol_per_apply_call"], apply_batch_cols=row["apply_batch_cols"], apply_streams=args.streams or 3,
-                                              apply_fft_path="pipeline kernel" if args.pipeline == 1 else "three kernels per batch", replicas=world),
+                                              apply_fft_path={1: "persistent pipeline kernel (TMA tiles, L2-resident k-space)", 2: "three kernels per batch, TMA-staged x kernel"}.get(args.pipeline, "library default: three kernels per batch (TMA-staged x kernel on 80/112/128 grids)"), replicas=world),
                 hx_pts_per_s=n * ng / t_apply, gram_tflops=flops_exec / t_gram / 1e12,
                 gram_tflops_note="executed FP64 flops / t (H_sub in full + upper tiles of S_sub, incl. tile padding); "
                                  "algorithmic (8*Ng*(n^2+n(n+1)/2)) = %.2f TF/s is roofline.achieved; the dense-equivalent 2*8*n^2*Ng count of SURVEY 8(d) "
@@ -653,7 +663,7 @@ def run_ours(args):
                                          note="rsdft_plan_set_gram_mode(1): H_sub upper tiles + conjugate mirror (30 % fewer flops). A production LOBPCG "
                                               "would run this mode (Hermitian eigen-solvers, rsdft_subspace_eig included, read one triangle); the headline keeps "
                                               "the full contraction because the definition and the paper's ZGEMM contract H_sub in full"),
-                next1_eig=eig, next2_rotate=rot, next2_rotate2=rot2,
+                apply_h_paths=paths, next1_eig=eig, next2_rotate=rot, next2_rotate2=rot2,
                 clocks=clocks, clocks_whole_run=all_clocks, e2e=e2e, gpu_launches=gpu_launches, cpu_baseline=cpu,
                 peaks_probe=peaks, library_yardstick=yard)
     line.update(extra)

@@ -24,9 +24,10 @@
 // and two ways to run them:
 //   * three kernels per column batch (fft3_fwd_zy_kernel, fft3_x_kernel, fft3_inv_yz_kernel): every kernel makes one
 //     HBM round trip of the batch;
-//   * ONE persistent kernel (fft3_pipeline_kernel) that walks (column, phase, tile) work items from an in-order queue
-//     with per-column completion counters, keeping about three columns of k-space in flight so that the hand-over
-//     fwd -> x -> inv goes through L2 instead of HBM (north_star "one HBM round trip per direction").
+//   * ONE persistent kernel (fft3_pipeline_kernel, fft3_tma_kernels.cuh) that walks (column, phase, tile) work items
+//     from an in-order queue with per-column completion counters, keeping about four columns of k-space in flight so
+//     that the hand-over fwd -> x -> inv goes through L2 instead of HBM (north_star "one HBM round
+//     trip per direction"); its tiles are TMA boxes in dense shared-memory slots.
 // The inverse transform is the forward codelet run on (im, re)-swapped data.
 // All global accesses are >= 64 B contiguous segments of 16 B elements.
 #pragma once
@@ -532,16 +533,15 @@ __global__ void __maxnreg__(((65536 / (NT * MINB)) / 8 * 8) > 255 ? 255 : ((6553
 }
 
 // ---------------------------------------------------------------------------------------------
-// The persistent pipeline: ONE launch applies T + V_loc to all `ncol` columns.  Work items (phase, column, tile)
-// are handed out in queue order by an atomic counter; the queue is built from "super-steps": super-step s holds the
-// fwd items of column s, the x items of column s-1 and the inv items of column s-2, interleaved by `pattern`
-// (one entry per item of a super-step: phase << 28 | tile).  An x item of column c needs ALL fwd items of c, an inv
-// item ALL x items of c: per-column completion counters `done[phase*ncol + c]`, waited on by a spin (dependencies
-// always sit earlier in the queue, and a CTA never waits while holding an earlier unfinished item, so the smallest
-// unfinished item always makes progress: no co-residency assumption, no deadlock).  About three columns of k-space
-// are in flight, so the k-space written by fwd is still in L2 when x and inv read it.
-// CTA = 256 threads: the x program runs one tile with all of them; the fwd and inv programs run TWO tiles side by side
-// (two 128-thread groups with their own named barrier and their own half of the shared memory).
+// Work queue of the persistent pipeline kernel (fft3_tma_kernels.cuh): ONE launch applies T + V_loc to all `ncol`
+// columns.  Work items (phase, column, tile) are handed out in queue order by an atomic counter; the queue is built
+// from "super-steps": super-step s holds the fwd items of column s, the x items of column s - lag_x and the inv items
+// of column s - lag_inv, interleaved by `pattern` (one entry per item of a super-step: phase << 28 | tile).  An x item
+// of column c needs ALL fwd items of c, an inv item ALL x items of c: per-column completion counters
+// `done[phase*ncol + c]` (dependencies always sit earlier in the queue, and nothing ever waits while holding an
+// earlier unfinished item, so the smallest unfinished item always makes progress: no co-residency assumption, no
+// deadlock).  About four columns of k-space are in flight, so the k-space written by fwd is still in L2 when x and
+// inv read it.
 struct PipeArgs {
     int32_t *head;           // queue position counter (zeroed before the launch)
     int32_t *done;           // [3][ncol] finished items per (phase, column) (zeroed before the launch)
@@ -552,85 +552,10 @@ struct PipeArgs {
     int32_t lag_x, lag_inv;      // super-step s holds fwd(s), x(s - lag_x), inv(s - lag_inv)
 };
 
-template <int N, int R2Y> struct PipeCfg {
-    static constexpr int TZ = XCfg<N>::TZ;
-    static constexpr size_t smem(int my)
-    {
-        const size_t zy = 2 * ZyCfg<N, R2Y>::SMEM_FWD;
-        const size_t x = (size_t)N * (my * TZ + 1) * sizeof(double2);
-        return zy > x ? zy : x;
-    }
-};
-
 __device__ __forceinline__ void pipe_wait(const int32_t *cnt, int want)
 {
     while (*((const volatile int32_t *)cnt) < want) __nanosleep(64);
     __threadfence();
-}
-
-template <int N, int R2Y>
-__global__ void __launch_bounds__(256, 2) fft3_pipeline_kernel(Fft3Args a, PipeArgs q)
-{
-    using C = ZyCfg<N, R2Y>;
-    constexpr int TZ = XCfg<N>::TZ, NT = 256, NH = 128;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2 *S = reinterpret_cast<double2 *>(smem_raw);
-    __shared__ double2 twz_s[C::NTWZ];           // z twiddles = x twiddles (cubic in x and z)
-    __shared__ double kinx_s[N];
-    __shared__ double2 twy_s[2][R2Y];
-    __shared__ int32_t next_item;
-    const int tid = threadIdx.x, half = tid >> 7, htid = tid & (NH - 1);
-    const int my = a.my;
-    fft3_x_tables<N, NT>(a, twz_s, kinx_s, tid);
-    const uint64_t pol_stream = l2_policy(a.hint_stream), pol_keep = l2_policy(a.hint_keep);
-    if (tid == 0) next_item = atomicAdd(q.head, 1);
-    __syncthreads();
-    const int64_t total = (int64_t)(a.ncol + q.lag_inv) * q.npattern;
-    for (;;) {
-        const int item = next_item;
-        __syncthreads();                                          // everyone has read next_item
-        if (item >= total) break;
-        if (tid == 0) next_item = atomicAdd(q.head, 1);           // its latency hides behind this item
-        const int s = item / q.npattern;
-        const uint32_t e = q.pattern[item - s * q.npattern];
-        const int ph = (int)(e >> 28), t = (int)(e & 0x0fffffffu);
-        const int col = s - (ph == 0 ? 0 : (ph == 1 ? q.lag_x : q.lag_inv));
-        if (col < 0 || col >= a.ncol) { __syncthreads(); continue; }
-        if (ph == 0) {
-            // two fwd tiles side by side: tile u = 2t + half -> (x, n2y) = (u / my, u % my)
-            const int u = 2 * t + half, x = u / my, n2y = u - x * my;
-            if (htid < R2Y) twy_s[half][htid] = a.twy[n2y * htid];
-            group_sync(1 + half, NH);
-            fft3_fwd_tile<N, R2Y, NH, true>(a.X + (int64_t)col * a.ldx + (int64_t)x * a.ny * N, a.W + (int64_t)col * a.ldw + (int64_t)x * a.ny * N,
-                                            my, n2y, S + half * C::TILE, twz_s, twy_s[half], htid, 1 + half, pol_stream, pol_keep);
-        } else if (ph == 1) {
-            if (tid == 0) pipe_wait(q.done + col, q.n_fwd);
-            __syncthreads();
-            const int k1y = t / q.zchunks, zc = t - k1y * q.zchunks;
-            const int64_t toff = (int64_t)(k1y * my) * a.nz + zc * TZ;
-            fft3_x_tile<N, TZ, NT, true>(a, a.W + (int64_t)col * a.ldw + toff, a.kin_yz + toff, S, twz_s, kinx_s, tid, pol_keep);
-        } else {
-            if (tid == 0) pipe_wait(q.done + a.ncol + col, q.n_x);
-            __syncthreads();
-            const int u = 2 * t + half, x = u / my, n2y = u - x * my;
-            if (htid < R2Y) twy_s[half][htid] = a.twy[n2y * htid];
-            const int64_t po = (int64_t)x * a.ny * N;
-            double2 *Sh = S + half * C::TILE;
-            fft3_issue_w_tile<N, R2Y, NH, true>(a.W + (int64_t)col * a.ldw + po, my, n2y, Sh, htid, pol_stream);     // cp.async.cg: L2 only; last use of the k-space lines
-            cp_async_commit();
-            cp_async_wait<0>();
-            group_sync(1 + half, NH);
-            fft3_inv_stages_12<N, R2Y, NH>(Sh, twy_s[half], htid, 1 + half);
-            group_sync(1 + half, NH);
-            fft3_inv_stage_3<N, R2Y, NH, false, true>(Sh, twz_s, nullptr, a.X + (int64_t)col * a.ldx + po, a.vloc + po,
-                                                      a.HX + (int64_t)col * a.ldhx + po, my, n2y, htid, pol_stream);
-        }
-        __syncthreads();                                          // all stores of this item are issued
-        if (tid == 0) {
-            __threadfence();
-            if (ph < 2) atomicAdd(q.done + ph * a.ncol + col, 1);
-        }
-    }
 }
 
 }  // namespace rsdft

@@ -115,8 +115,7 @@ struct rsdft_plan {
     // apply_h batching
     int batch = 0;                // columns per kernel sequence
     int user_batch = 0;
-    int pipeline = 0;             // 1: persistent FFT pipeline kernel where available (rsdft_plan_set_pipeline)
-    int x_tma = 1;                // 1: TMA-staged x kernel where the shape has one
+    int pipeline = 3;             // FFT path (rsdft_plan_set_pipeline): 0 three kernels, 1 persistent pipeline kernel, 2 three kernels with the TMA-staged x kernel, 3 auto
     DevBuf<uint32_t> pipe_pattern;
     DevBuf<int32_t> pipe_counters;
     int pipe_key = -1, pipe_npattern = 0;
@@ -533,10 +532,9 @@ bool x_tile_map(CUtensorMap *tm, const Fft3Args &a, int tz)
     const cuuint64_t gstr[3] = {(cuuint64_t)a.nz * 16, (cuuint64_t)a.ny * a.nz * 16, (cuuint64_t)a.ldw * 16};
     const cuuint32_t box[4] = {(cuuint32_t)(2 * tz), (cuuint32_t)a.my, (cuuint32_t)a.nx, 1};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
-    if (const char *e = getenv("RSDFT_LAB_PROMO")) promo = atoi(e) == 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : (atoi(e) == 64 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : (atoi(e) == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : promo));   // LAB
+    // (L2 promotion 64 / 128 / 256 B: no measurable difference on the x tile)
     return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)a.W, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // TMA-staged x kernel (fft3_tma_kernels.cuh); returns cudaErrorNotSupported when the shape has none
@@ -565,13 +563,11 @@ cudaError_t launch_x_tma(const Fft3Args &a, int sms, cudaStream_t st)
 #ifdef RSDFT_LAB_N
         if (const char *e = getenv("RSDFT_LAB_XCFG")) {
             switch (atoi(e)) {
-            case 1: return launch_x_tma_cfg<NX, 4, 6, 96, 1>(a, sms, st);
-            case 2: return launch_x_tma_cfg<NX, 4, 3, 96, 2>(a, sms, st);
-            case 3: return launch_x_tma_cfg<NX, 4, 5, 96, 1>(a, sms, st);
-            case 4: return launch_x_tma_cfg<NX, 4, 4, 160, 1>(a, sms, st);
-            case 5: return launch_x_tma_cfg<NX, 8, 2, 160, 1>(a, sms, st);
-            case 6: return launch_x_tma_cfg<NX, 8, 3, 160, 1>(a, sms, st);
-            case 7: return launch_x_tma_cfg<NX, 4, 6, 64, 1>(a, sms, st);
+            case 1: return launch_x_tma_cfg<NX, 8, 2, 160, 1>(a, sms, st);
+            case 2: return launch_x_tma_cfg<NX, 8, 2, 128, 1>(a, sms, st);
+            case 3: return launch_x_tma_cfg<NX, 8, 2, 96, 1>(a, sms, st);
+            case 4: return launch_x_tma_cfg<NX, 8, 2, 288, 1>(a, sms, st);
+            case 5: return launch_x_tma_cfg<NX, 8, 3, 160, 1>(a, sms, st);
             default: break;
             }
         }
@@ -595,28 +591,70 @@ cudaError_t launch_x(const Fft3Args &a, int sms, cudaStream_t st)
     return launch_x_cfg<NX, 2, 256, 1>(a, sms, st);
 }
 
-// the persistent pipeline kernel exists for cubic grids of these lengths (the shapes of the five configs and of
-// the paper's two grids); everything else runs the three-kernel path
+// Shapes of the persistent pipeline kernel (fft3_tma_kernels.cuh): cubic grids with a radix-16 first stage whose
+// regions fit the 227 KB of shared memory.  TZ = z points per x tile, NS = fwd / inv slots per group.
+template <int N> struct PipeShape { static constexpr int TZ = 0, NS = 0; };
+template <> struct PipeShape<48> { static constexpr int TZ = 8, NS = 3; };
+template <> struct PipeShape<64> { static constexpr int TZ = 8, NS = 3; };
+template <> struct PipeShape<80> { static constexpr int TZ = 8, NS = 3; };
+template <> struct PipeShape<96> { static constexpr int TZ = 8, NS = 3; };
+template <> struct PipeShape<112> { static constexpr int TZ = 4, NS = 2; };
+template <> struct PipeShape<128> { static constexpr int TZ = 4, NS = 2; };
+template <int N> constexpr int pipe_tz() { return PipeShape<N>::TZ; }
+
+// tensor maps of the pipeline kernel
+bool rows_map(CUtensorMap *tm, const void *base, int64_t ld, const Fft3Args &a)
+{
+    TmaEncodeFn enc = tma_encoder();
+    if (!enc || ((uintptr_t)base & 15) != 0 || 2 * a.nz > 256) return false;
+    const cuuint64_t gdim[5] = {(cuuint64_t)2 * a.nz, (cuuint64_t)a.my, (cuuint64_t)a.r2y, (cuuint64_t)a.nx, (cuuint64_t)a.ncol};
+    const cuuint64_t gstr[4] = {(cuuint64_t)a.nz * 16, (cuuint64_t)a.my * a.nz * 16, (cuuint64_t)a.ny * a.nz * 16, (cuuint64_t)ld * 16};
+    const cuuint32_t box[5] = {(cuuint32_t)(2 * a.nz), 1, (cuuint32_t)a.r2y, 1, 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<void *>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+bool vrows_map(CUtensorMap *tm, const Fft3Args &a)
+{
+    TmaEncodeFn enc = tma_encoder();
+    if (!enc || ((uintptr_t)a.vloc & 15) != 0 || a.nz > 256 || (a.nz & 1)) return false;
+    const cuuint64_t gdim[4] = {(cuuint64_t)a.nz, (cuuint64_t)a.my, (cuuint64_t)a.r2y, (cuuint64_t)a.nx};
+    const cuuint64_t gstr[3] = {(cuuint64_t)a.nz * 8, (cuuint64_t)a.my * a.nz * 8, (cuuint64_t)a.ny * a.nz * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)a.nz, 1, (cuuint32_t)a.r2y, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(a.vloc), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 template <int N>
 cudaError_t launch_pipeline(const Fft3Args &a, const PipeArgs &q, int sms, cudaStream_t st)
 {
-    constexpr int R2 = Axis<N>::R2;
-    auto k = fft3_pipeline_kernel<N, R2>;
-    const size_t smem = PipeCfg<N, R2>::smem(a.my);
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    const int64_t total = (int64_t)(a.ncol + q.lag_inv) * q.npattern;
-    k<<<(int)std::min<int64_t>(total, (int64_t)sms * 2), 256, smem, st>>>(a, q);
-    return cudaSuccess;
+    using Sh = PipeShape<N>;
+    if constexpr (Sh::TZ == 0) {
+        return cudaErrorNotSupported;
+    } else {
+        constexpr int G = 3, NTG = 96;
+        PipeMaps maps;
+        if (!rows_map(&maps.x_rows, a.X, a.ldx, a) || !rows_map(&maps.w_rows, a.W, a.ldw, a) || !x_tile_map(&maps.w_xtile, a, Sh::TZ) ||
+            !vrows_map(&maps.v_rows, a))
+            return cudaErrorNotSupported;
+        auto k = fft3_pipeline_kernel<N, 16, Sh::TZ, Sh::NS, G, NTG>;
+        const size_t smem = (size_t)G * PipeCfg<N, 16, Sh::TZ, Sh::NS>::REGION + 1024;
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        const int64_t total = (int64_t)(a.ncol + q.lag_inv) * q.npattern;
+        k<<<(int)std::min<int64_t>((total + G - 1) / G, (int64_t)sms), G * (NTG + 64), smem, st>>>(a, q, maps);
+        return cudaSuccess;
+    }
 }
+
 #ifdef RSDFT_LAB_N
 #define RS_PIPE_LENGTHS(X_) X_(RSDFT_LAB_N)
 #else
-#define RS_PIPE_LENGTHS(X_) X_(48) X_(60) X_(64) X_(80) X_(96) X_(112) X_(128)
+#define RS_PIPE_LENGTHS(X_) X_(48) X_(64) X_(80) X_(96) X_(112) X_(128)
 #endif
 inline bool pipeline_available(const int n[3])
 {
-    if (n[0] != n[1] || n[1] != n[2]) return false;
+    if (n[0] != n[1] || n[1] != n[2] || !tma_encoder()) return false;
 #define RS_PIPE_OK(N_) case N_: return true;
     switch (n[0]) { RS_PIPE_LENGTHS(RS_PIPE_OK) default: return false; }
 #undef RS_PIPE_OK
@@ -677,11 +715,13 @@ Fft3Args fft3_args(const rsdft_plan *P, int nb, const double2 *X, int64_t ldx, d
     fa.r2y = first_radix(P->n[1]); fa.my = P->n[1] / fa.r2y;
     fa.twx = P->tw[0].p; fa.twy = P->tw[1].p; fa.twz = P->tw[2].p;
     fa.kin_x = P->kin_x.p; fa.kin_yz = P->kin_yz.p; fa.vloc = P->vloc.p;
-    fa.hint_stream = 1; fa.hint_keep = 0;
-    fa.x_tma = P->x_tma;
-    if (const char *e = getenv("RSDFT_LAB_XTMA")) fa.x_tma = atoi(e);   // LAB
-    if (getenv("RSDFT_LAB_XNOSTORE")) fa.x_tma |= 2;   // LAB
-    if (const char *e = getenv("RSDFT_LAB_HINTS")) { fa.hint_stream = (e[0] - '0'); fa.hint_keep = (e[1] - '0'); }   // LAB
+    fa.hint_stream = 1; fa.hint_keep = 0;       // measured: X / psi / HX evict_first halves the pipeline kernel's DRAM traffic; evict_last on k-space adds nothing
+    // auto (3): the TMA x kernel where it measured faster end to end (80^3 -7 %, 112^3 -6 %, 128^3 -7 %; 96^3 +2 %)
+    fa.x_tma = P->pipeline == 2 || (P->pipeline == 3 && (P->n[0] == 80 || P->n[0] == 112 || P->n[0] == 128));
+#ifdef RSDFT_LAB_N
+    if (const char *e = getenv("RSDFT_LAB_XTMA")) fa.x_tma = atoi(e);
+    if (const char *e = getenv("RSDFT_LAB_HINTS")) { fa.hint_stream = (e[0] - '0'); fa.hint_keep = (e[1] - '0'); }
+#endif
     return fa;
 }
 
@@ -733,7 +773,7 @@ int apply_h_batch(rsdft_plan *P, int slot, int nb, int fft_batch, const double2 
 // item order inside one super-step of the pipeline queue: the three phases interleaved in proportion
 int pipeline_pattern(rsdft_plan *P, const Fft3Args &fa, int tz, PipeArgs &q, cudaStream_t st)
 {
-    q.n_fwd = fa.nx * fa.my / 2;
+    q.n_fwd = fa.nx * fa.my;
     q.zchunks = fa.nz / tz;
     q.n_x = fa.r2y * q.zchunks;
     q.n_inv = q.n_fwd;
@@ -760,8 +800,11 @@ int pipeline_pattern(rsdft_plan *P, const Fft3Args &fa, int tz, PipeArgs &q, cud
     q.pattern = P->pipe_pattern.p;
     q.npattern = P->pipe_npattern;
     q.lag_x = 1;
-    q.lag_inv = 3;
-    if (const char *e = getenv("RSDFT_LAB_LAG")) q.lag_inv = atoi(e);   // LAB      // measured at configs[2]: lag 2 -> 38.6 ms, 3 -> 36.8, 4 -> 36.9 per 1440 columns
+    q.lag_inv = 3;      // measured at configs[2] (FFT only, us per column): lag 2 -> 23.2, 3 -> 17.6, 4 -> 17.7; lag_x 2 / lag_inv 4 -> 18.3
+#ifdef RSDFT_LAB_N
+    if (const char *e = getenv("RSDFT_LAB_LAG")) q.lag_inv = atoi(e);
+    if (const char *e = getenv("RSDFT_LAB_LAGX")) q.lag_x = atoi(e);
+#endif
     return RSDFT_OK;
 }
 
@@ -784,7 +827,7 @@ int apply_h_pipeline(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, dou
     const Fft3Args fa = fft3_args(P, ncol, X, ldx, HX, ldhx);
     PipeArgs q;
     int tz = 0;
-#define RS_PIPE_TZ(N_) case N_: tz = XCfg<N_>::TZ; break;
+#define RS_PIPE_TZ(N_) case N_: tz = pipe_tz<N_>(); break;
     switch (P->n[0]) { RS_PIPE_LENGTHS(RS_PIPE_TZ) default: break; }
 #undef RS_PIPE_TZ
     if (int rc = pipeline_pattern(P, fa, tz, q, st)) return rc;
@@ -811,7 +854,7 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
 {
     const int batch = P->user_batch > 0 ? P->user_batch : default_batch(P);
     P->batch = batch;
-    if (P->pipeline && pipeline_available(P->n)) return apply_h_pipeline(P, ncol, X, ldx, HX, ldhx, batch, st);
+    if (P->pipeline == 1 && pipeline_available(P->n)) return apply_h_pipeline(P, ncol, X, ldx, HX, ldhx, batch, st);
     // With large projector tables (configs 3, 4: 43 / 98 MB of beta) the projector kernels work on units of 4 FFT
     // batches: project and scatter read beta once per unit, so its traffic per column drops 4x.
     const bool big_beta = P->natom > 0 && P->beta.bytes() >= ((size_t)32 << 20);
@@ -1077,7 +1120,7 @@ int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols)
 
 int rsdft_plan_set_pipeline(rsdft_plan_t *plan, int32_t mode)
 {
-    if (!plan || (mode != 0 && mode != 1)) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_pipeline: mode must be 0 or 1");
+    if (!plan || mode < 0 || mode > 3) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_pipeline: mode must be 0 ... 3");
     plan->pipeline = mode;
     return RSDFT_OK;
 }

@@ -131,9 +131,10 @@ def test_lengths_with_first_radix_12(env, n3):
 
 @pytest.mark.parametrize("N,ncol", [(48, 13), (60, 9), (64, 7), (80, 5), (96, 7), (112, 4), (128, 3)])
 def test_pipeline_kernel_matches_three_kernel_path(env, N, ncol):
-    """rsdft_plan_set_pipeline(1): the persistent FFT kernel (work queue + per-column completion counters) gives the
-    same bits as the three-kernel path, on a caller's side stream, with overlapping projector spheres; and both match
-    the oracle on sampled columns."""
+    """rsdft_plan_set_pipeline(1): the persistent FFT kernel (work queue, per-column completion counters, TMA boxes issued
+    by control warps) and rsdft_plan_set_pipeline(2): the TMA-staged x kernel give the same bits as the three-kernel
+    path, on a caller's side stream, with overlapping projector spheres; and they match the oracle on sampled columns.
+    (60 = 12*5 has no pipeline kernel: the call silently runs path 0.)"""
     torch, oracle, rsdft, wl = env["torch"], env["oracle"], env["rsdft"], env["wl"]
     L = (0.22 * N,) * 3
     system = wl.small_system(n=(N, N, N), L=L, natom=6, seed=N, nproj=4, rc=1.8)
@@ -141,10 +142,10 @@ def test_pipeline_kernel_matches_three_kernel_path(env, N, ncol):
     plan = rsdft.plan_from_system(system)
     X = wl.orbital_block(ng, range(ncol), 31, 0, device="cuda", ld=ng + 16)
     ref = gpu_apply(env, plan, X)
-    rsdft.rsdft_plan_set_pipeline(plan, 1)
     side = torch.cuda.Stream()
     outs = []
-    for batch in (0, 2):
+    for mode, batch in ((1, 0), (1, 2), (2, 0), (2, 2)):
+        rsdft.rsdft_plan_set_pipeline(plan, mode)
         rsdft.rsdft_plan_set_batch(plan, batch)
         with torch.cuda.stream(side):
             HX = torch.full_like(X, float("nan"))
