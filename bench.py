@@ -471,7 +471,7 @@ def run_ours(args):
     for mode, name in ((0, "three_kernels"), (1, "pipeline_kernel"), (2, "three_kernels_tma_x")):
         rsdft.rsdft_plan_set_pipeline(plan, mode)
         paths[name + "_ms"] = 1e3 * timed(torch, lambda: rsdft.rsdft_apply_h(plan, Y, HY), 2)
-    rsdft.rsdft_plan_set_pipeline(plan, args.pipeline if args.pipeline >= 0 else 3)
+    rsdft.rsdft_plan_set_pipeline(plan, args.pipeline if args.pipeline >= 0 else 2)
     paths["note"] = ("rsdft_plan_set_pipeline 0 / 1 / 2 on the headline block, ms per apply_h call; bitwise identical results (tests); "
                      "the pipeline kernel keeps k-space in L2 (58 B of DRAM traffic per orbital*point against 112) but is bound by the "
                      "SM's L1/shared-memory data pipe, see DESIGN.md")
@@ -651,7 +651,7 @@ def run_ours(args):
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64 (complex128)",
                 data="synthetic", config=dict(workload=workload_name(args.config), l2="inputs %.1f GB per block >> 126 MB L2, no flush needed" % (n * ng * 16 / 1e9),
                                               ncol_per_apply_call=row["ncol_per_apply_call"], apply_batch_cols=row["apply_batch_cols"], apply_streams=args.streams or 3,
-                                              apply_fft_path={1: "persistent pipeline kernel (TMA tiles, L2-resident k-space)", 2: "three kernels per batch, TMA-staged x kernel"}.get(args.pipeline, "library default: three kernels per batch (TMA-staged x kernel on 80/112/128 grids)"), replicas=world),
+                                              apply_fft_path={1: "persistent pipeline kernel (TMA tiles, L2-resident k-space)", 2: "three kernels per batch, TMA-staged x kernel"}.get(args.pipeline if args.pipeline >= 0 else 2, "three kernels per batch"), replicas=world),
                 hx_pts_per_s=n * ng / t_apply, gram_tflops=flops_exec / t_gram / 1e12,
                 gram_tflops_note="executed FP64 flops / t (H_sub in full + upper tiles of S_sub, incl. tile padding); "
                                  "algorithmic (8*Ng*(n^2+n(n+1)/2)) = %.2f TF/s is roofline.achieved; the dense-equivalent 2*8*n^2*Ng count of SURVEY 8(d) "

@@ -204,13 +204,14 @@ int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols);
  * Errors: INVALID_ARG. */
 int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams);
 
-/* apply_h FFT path.  0: three FFT kernels per column batch (every kernel makes one HBM round trip of the batch).
- * 1: ONE persistent kernel per call that walks (column, phase, tile) work items in dependency order so that the
- * k-space of about four columns stays in L2 between the forward, x and inverse programs; every tile is a TMA box
- * (cp.async.bulk.tensor) fetched ahead of the compute warps by control warps; available for cubic grids of length
- * 48, 64, 80, 96, 112, 128 (other grids silently use path 0).  2: path 0 with the TMA-staged x kernel (grids with
- * nx = ny of those lengths).  3 (default): path 0, with the TMA-staged x kernel on the lengths where it measured
- * faster end to end (80, 112, 128).  Results are bitwise identical on all paths.
+/* apply_h FFT path.  0: three FFT kernels per column batch (every kernel makes one HBM round trip of the batch), tiles
+ * loaded by the threads.  2 (default): the same three kernels, but the x kernel fetches its tile as one TMA box
+ * (cp.async.bulk.tensor) into a dense shared-memory slot and runs its radix stages in place, the two radix-M stage
+ * pairs fused in registers for lengths <= 96 (grids with nx = ny in {48, 64, 80, 96, 112, 128}; other grids silently
+ * use path 0).  1: ONE persistent kernel per call that walks (column, phase, tile) work items in dependency order so
+ * that the k-space of about four columns stays in L2 between the forward, x and inverse programs; every tile is a
+ * TMA box fetched ahead of the compute warps by control warps (cubic grids of those lengths, else path 2 / 0).
+ * Results are bitwise identical on all paths.
  * Errors: INVALID_ARG. */
 int rsdft_plan_set_pipeline(rsdft_plan_t *plan, int32_t mode);
 

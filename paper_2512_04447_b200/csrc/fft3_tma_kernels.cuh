@@ -132,6 +132,93 @@ __device__ __forceinline__ void fft3_x_dense_tile(const Fft3Args &a, double2 *S,
     }
 }
 
+// Same tile with the two radix-M stage pairs fused in registers: a thread holds the M x M block (n1, jy) of one
+// (n2, z), runs the M y-transforms and the M x-transforms (stage A) on it without going through shared memory, and does
+// the mirror image on the way out.  Two of the four shared-memory exchanges disappear (the tile is bound by the
+// L1/shared-memory data pipe): 96 B per point of LDS/STS traffic instead of 160.  2*M*M doubles of
+// registers per thread, so M <= 6 (lengths <= 96) and at most 256 threads per CTA.
+template <int NX, int TZ, int NTG, bool HINT>
+__device__ __forceinline__ void fft3_x_dense_tile_fused(const Fft3Args &a, double2 *S, double2 *gbase, const double *__restrict__ kin,
+                                                        const double2 *twx_s, const double *kinx_s, int tid, int bar, uint64_t pol)
+{
+    using D = XDense<NX, TZ>;
+    constexpr int R2X = D::R2X, M = D::MX, LINES = D::LINES;
+    static_assert(M <= 6, "fused x tile: register block is 2*M*M doubles");
+    // y stage B + x stage A
+    for (int item = tid; item < TZ * R2X; item += NTG) {
+        const int z = item % TZ, n2 = item / TZ;
+        double2 *p = S + n2 * LINES + z;
+        double re[M][M], im[M][M];                   // [n1][jy]
+#pragma unroll
+        for (int n1 = 0; n1 < M; ++n1)
+#pragma unroll
+            for (int j = 0; j < M; ++j) { const double2 v = p[n1 * R2X * LINES + j * TZ]; re[n1][j] = v.x; im[n1][j] = v.y; }
+#pragma unroll
+        for (int n1 = 0; n1 < M; ++n1) Dft<M>::run(re[n1], im[n1]);
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+            double cr[M], ci[M];
+#pragma unroll
+            for (int n1 = 0; n1 < M; ++n1) { cr[n1] = re[n1][j]; ci[n1] = im[n1][j]; }
+            Dft<M>::run(cr, ci);
+#pragma unroll
+            for (int k = 1; k < M; ++k) { const double2 w = twx_s[(k - 1) * R2X + n2]; tw_mul(cr[k], ci[k], w.x, -w.y); }
+#pragma unroll
+            for (int k = 0; k < M; ++k) p[k * R2X * LINES + j * TZ] = make_double2(cr[k], ci[k]);
+        }
+    }
+    group_sync(bar, NTG);
+    // x stage B (radix-R2X over n2) -> frequency kx = k1 + M*k2; kinetic factor; inverse stage B'
+    constexpr int XB_ITEMS = LINES * M;
+    constexpr int XB_NT = (XB_ITEMS % NTG == 0) ? NTG : ((XB_ITEMS % 96 == 0 && NTG > 96) ? 96 : NTG);
+    for (int item = tid; item < XB_ITEMS && tid < XB_NT; item += XB_NT) {
+        const int line = item % LINES, k1 = item / LINES;
+        double2 *p = S + k1 * R2X * LINES + line;
+        const int jy = line / TZ, z = line - jy * TZ;
+        const double tin = __ldg(kin + (int64_t)jy * a.nz + z);
+        double br[R2X], bi[R2X];
+#pragma unroll
+        for (int t = 0; t < R2X; ++t) { const double2 v = p[t * LINES]; br[t] = v.x; bi[t] = v.y; }
+        Dft<R2X>::run(br, bi);
+#pragma unroll
+        for (int k2 = 0; k2 < R2X; ++k2) {
+            const double f = kinx_s[k1 + M * k2] + tin;
+            br[k2] *= f; bi[k2] *= f;
+        }
+        Dft<R2X>::run(bi, br);                  // swapped domain from here on
+#pragma unroll
+        for (int t = 0; t < R2X; ++t) p[t * LINES] = make_double2(br[t], bi[t]);
+    }
+    group_sync(bar, NTG);
+    // x inverse stage A' + y inverse stage B' + store
+    for (int item = tid; item < TZ * R2X; item += NTG) {
+        const int z = item % TZ, n2 = item / TZ;
+        const double2 *p = S + n2 * LINES + z;
+        double re[M][M], im[M][M];                   // [jy][k -> n1]
+#pragma unroll
+        for (int j = 0; j < M; ++j) {
+#pragma unroll
+            for (int k = 0; k < M; ++k) { const double2 v = p[k * R2X * LINES + j * TZ]; re[j][k] = v.x; im[j][k] = v.y; }
+#pragma unroll
+            for (int k = 1; k < M; ++k) { const double2 w = twx_s[(k - 1) * R2X + n2]; tw_mul(im[j][k], re[j][k], w.x, -w.y); }
+            Dft<M>::run(im[j], re[j]);
+        }
+#pragma unroll
+        for (int n1 = 0; n1 < M; ++n1) {
+            double cr[M], ci[M];
+#pragma unroll
+            for (int j = 0; j < M; ++j) { cr[j] = re[j][n1]; ci[j] = im[j][n1]; }
+            Dft<M>::run(ci, cr);
+            double2 *ptr = gbase + (int64_t)(n1 * R2X + n2) * a.ny * a.nz + z;
+#pragma unroll
+            for (int j = 0; j < M; ++j) {
+                if (HINT) st_hint(ptr + (int64_t)j * a.nz, make_double2(cr[j], ci[j]), pol);
+                else ptr[(int64_t)j * a.nz] = make_double2(cr[j], ci[j]);
+            }
+        }
+    }
+}
+
 // Launch shape per length: z points per tile, groups per CTA, threads per group, slots per group.
 // NTG is chosen so that the heaviest stage (LINES*MX radix-16 pairs) fills whole rounds.
 template <int NX> struct XTmaCfg { static constexpr int TZ = 0, G = 0, NTG = 0, SPG = 0; };      // TZ = 0: no TMA kernel for this length
@@ -193,7 +280,10 @@ __global__ void __launch_bounds__(G * NTG, 1) fft3_x_tma_kernel(Fft3Args a, cons
         decode(tile, col, k1y, zc);
         const int64_t toff = (int64_t)(k1y * my) * a.nz + zc * TZ;
         double2 *S = reinterpret_cast<double2 *>(slots + (size_t)(g * SPG + slot) * D::SLOT);
-        fft3_x_dense_tile<NX, TZ, NTG, false>(a, S, a.W + col * a.ldw + toff, a.kin_yz + toff, twx_s, kinx_s, gt, 1 + g, pol);
+        if constexpr (D::MX <= 6)
+            fft3_x_dense_tile_fused<NX, TZ, NTG, false>(a, S, a.W + col * a.ldw + toff, a.kin_yz + toff, twx_s, kinx_s, gt, 1 + g, pol);
+        else
+            fft3_x_dense_tile<NX, TZ, NTG, false>(a, S, a.W + col * a.ldw + toff, a.kin_yz + toff, twx_s, kinx_s, gt, 1 + g, pol);
         fence_proxy_async_smem();
         group_sync(1 + g, NTG);                       // the slot is free: every thread has finished reading it
         if (SPG == 1 && gt == 0 && tile + stride < ntiles) issue(tile + stride, 0);

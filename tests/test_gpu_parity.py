@@ -141,6 +141,7 @@ def test_pipeline_kernel_matches_three_kernel_path(env, N, ncol):
     ng = N ** 3
     plan = rsdft.plan_from_system(system)
     X = wl.orbital_block(ng, range(ncol), 31, 0, device="cuda", ld=ng + 16)
+    rsdft.rsdft_plan_set_pipeline(plan, 0)
     ref = gpu_apply(env, plan, X)
     side = torch.cuda.Stream()
     outs = []
@@ -261,7 +262,7 @@ def test_repeated_calls_are_bitwise_reproducible(env):
     Y = wl.orbital_block(ng, range(60), 19, 0, device="cuda")
     ref = None
     for rep in range(5):
-        rsdft.rsdft_plan_set_pipeline(plan, rep % 2)
+        rsdft.rsdft_plan_set_pipeline(plan, rep % 3)
         HY = torch.full_like(Y, float("nan"))
         rsdft.rsdft_apply_h(plan, Y, HY)
         H, S = rsdft.rsdft_subspace_gram(plan, Y, HY)
