@@ -194,7 +194,7 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
 int rsdft_plan_info(const rsdft_plan_t *plan, int64_t *out8);
 
 /* Tuning knob: number of columns apply_h pushes through its kernel sequence at a time
- * (0 = library default: about 270 MB of orbitals per launch). */
+ * (0 = library default: about 540 MB of orbitals per launch). */
 int rsdft_plan_set_batch(rsdft_plan_t *plan, int32_t batch_cols);
 
 /* Tuning knob: apply_h deals its column batches round-robin to `nstreams` plan-owned CUDA streams

@@ -568,7 +568,7 @@ cudaError_t launch_x_tma(const Fft3Args &a, int sms, cudaStream_t st)
             case 2: return launch_x_tma_cfg<NX, 8, 2, 128, 1>(a, sms, st);
             case 3: return launch_x_tma_cfg<NX, 8, 2, 96, 1>(a, sms, st);
             case 4: return launch_x_tma_cfg<NX, 8, 2, 288, 1>(a, sms, st);
-            case 5: return launch_x_tma_cfg<NX, 8, 3, 160, 1>(a, sms, st);
+            case 5: return launch_x_tma_cfg<NX, 8, 3, 96, 1>(a, sms, st);
             default: break;
             }
         }
@@ -669,7 +669,17 @@ void launch_project_mt(const SphereTables &t, const double2 *X, int64_t ldx, int
     // kernel is latency-bound on its gathers, so warps in flight matter more than reuse
     const int gx = (t.nchunks + 3) / 4;
     const int64_t want = (int64_t)sms * 8;
-    if (ncol > 16 && (int64_t)gx * ((ncol + 31) / 32) >= want)
+#ifdef RSDFT_LAB_N
+    if (const char *e = getenv("RSDFT_LAB_PG8")) {
+        const int g8 = atoi(e);
+        if (g8 == 4) project_kernel<MT, 4><<<dim3(gx, (ncol + 31) / 32), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+        else if (g8 == 2) project_kernel<MT, 2><<<dim3(gx, (ncol + 15) / 16), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+        else project_kernel<MT, 1><<<dim3(gx, (ncol + 7) / 8), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
+        return;
+    }
+#endif
+    // (two 8-row projector tiles with 32 columns per warp need 140 registers: 12 warps per SM; 16 columns measured 2 % faster at config 4)
+    if (MT == 1 && ncol > 16 && (int64_t)gx * ((ncol + 31) / 32) >= want)
         project_kernel<MT, 4><<<dim3(gx, (ncol + 31) / 32), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
     else if (ncol > 8 && (int64_t)gx * ((ncol + 15) / 16) >= want)
         project_kernel<MT, 2><<<dim3(gx, (ncol + 15) / 16), 128, 0, st>>>(t, X, ldx, ncol, dV, pp);
@@ -700,12 +710,12 @@ SphereTables sphere_tables(const rsdft_plan *P)
 
 int default_batch(const rsdft_plan *P)
 {
-    // columns per kernel sequence: ~270 MB of orbitals per launch (19 / 12 / 8 columns at 96^3 / 112^3 / 128^3).  Measured on B200 (configs 2-4): the
-    // kernels need >= 10-20 M points per launch to reach their asymptotic rate, and the k-space scratch
-    // stops being L2-resident beyond ~4 columns of 96^3 anyway, so small L2-sized batches only lose.
+    // columns per kernel sequence: ~540 MB of orbitals per launch (38 / 24 / 16 columns at 96^3 / 112^3 / 128^3, 68 at 80^3).  Measured on B200
+    // (configs 2-4, 80^3): the kernels need >= 10-20 M points per launch to reach their asymptotic rate, the k-space scratch stops being
+    // L2-resident beyond ~4 columns of 96^3 anyway (small L2-sized batches only lose), and 540 MB is 0-5 % faster than 270 MB.
     const int64_t per_col = P->ng * 16;
-    int64_t b = (int64_t)(270ll << 20) / per_col;
-    return (int)std::max<int64_t>(1, std::min<int64_t>(b, 64));
+    int64_t b = (int64_t)(540ll << 20) / per_col;
+    return (int)std::max<int64_t>(1, std::min<int64_t>(b, 96));
 }
 
 Fft3Args fft3_args(const rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx)
