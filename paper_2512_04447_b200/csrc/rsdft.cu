@@ -715,7 +715,7 @@ int default_batch(const rsdft_plan *P)
     // L2-resident beyond ~4 columns of 96^3 anyway (small L2-sized batches only lose), and 540 MB is 0-5 % faster than 270 MB.
     const int64_t per_col = P->ng * 16;
     int64_t b = (int64_t)(540ll << 20) / per_col;
-    return (int)std::max<int64_t>(1, std::min<int64_t>(b, 96));
+    return (int)std::max<int64_t>(1, std::min<int64_t>(b, 72));      // (small grids: 64-72 columns measured better than 96)
 }
 
 Fft3Args fft3_args(const rsdft_plan *P, int nb, const double2 *X, int64_t ldx, double2 *HX, int64_t ldhx)
@@ -921,7 +921,15 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
 }
 
 // Gram configuration: 96 x 96 complex tile, 8 warps (2 x 4), each 48 x 24 = 6 x 3 DMMA tiles
-using GCfg = GramCfg<2, 4, 6, 3, 16, 3>;
+#ifndef RSDFT_GRAM_WGM      // warps along M, warps along N, fragments per warp along M, along N, stages
+#define RSDFT_GRAM_WGM 2
+#define RSDFT_GRAM_WGN 4
+#define RSDFT_GRAM_FA 6
+#define RSDFT_GRAM_FB 3
+#define RSDFT_GRAM_STAGES 3
+#endif
+#define RSDFT_GRAM_SHAPE RSDFT_GRAM_WGM, RSDFT_GRAM_WGN, RSDFT_GRAM_FA, RSDFT_GRAM_FB, 16, RSDFT_GRAM_STAGES
+using GCfg = GramCfg<RSDFT_GRAM_SHAPE>;
 constexpr int GRAM_KC = 16;
 
 int choose_kslabs(int64_t ntiles, int64_t nchunks, int sms)
@@ -953,7 +961,7 @@ int gram_launch(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const doubl
     a.Y = Y; a.HY = HY; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = ntiles; a.kslabs = ks;
     a.nchunks = nchunks; a.tiles = dtiles; a.work = P->gram_work.p;
     // operand staging: TMA bulk copies (gram_bulk, rsdft_plan_set_gram_mode) or per-thread cp.async
-    auto kern = P->gram_bulk ? gram_dmma_kernel<2, 4, 6, 3, 16, 3, true> : gram_dmma_kernel<2, 4, 6, 3, 16, 3, false>;
+    auto kern = P->gram_bulk ? gram_dmma_kernel<RSDFT_GRAM_SHAPE, true> : gram_dmma_kernel<RSDFT_GRAM_SHAPE, false>;
     // the attribute is per device/context: set it on every launch (cheap), never cache it per thread
     RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
     kern<<<ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);

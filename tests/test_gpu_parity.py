@@ -485,6 +485,17 @@ def test_full_size_block_step_sampled_parity(env, cfg):
     hd = rows(lambda a, b: (Y[a:b].conj() * HY[a:b]).sum(dim=1))       # diag(H_sub) = <y_i | H y_i>
     assert np.max(np.abs(np.diagonal(Hg) - hd)) <= 1e-12 * scale_h
     np.linalg.cholesky(Sg)
+    # the other FFT paths at full size: three plain kernels and the persistent pipeline kernel (where the grid has one)
+    # rewrite the same HY bit for bit -- compared through per-column integer checksums of the bit patterns, so that no
+    # third block has to be resident
+    bits = lambda T: torch.view_as_real(T).view(torch.int64).sum(dim=(1, 2))
+    ref_bits = bits(HY)
+    for mode in (0, 1):
+        rsdft.rsdft_plan_set_pipeline(plan, mode)
+        HY.fill_(float("nan"))
+        rsdft.rsdft_apply_h(plan, Y, HY)
+        torch.cuda.synchronize()
+        assert torch.equal(bits(HY), ref_bits), "FFT path %d differs from the default path at full size" % mode
     plan.close()
 
 
