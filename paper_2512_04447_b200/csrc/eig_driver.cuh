@@ -183,7 +183,7 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
     const size_t smem_sub = (size_t)2 * D * (D + 1) * sizeof(double2);
     const size_t smem_upd = (size_t)3 * D * (D + 4) * sizeof(double2);
     RS_CUDA(cudaFuncSetAttribute(rsdft::jacobi_subeig_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_sub));
-    RS_CUDA(cudaFuncSetAttribute(rsdft::jacobi_colupdate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_upd));
+    RS_CUDA(cudaFuncSetAttribute(rsdft::jacobi_block_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_upd));
     double host[3] = {0.0, 0.0, 0.0};
     RS_CUDA(cudaMemcpyAsync(host, scal, sizeof(double), cudaMemcpyDeviceToHost, st));
     RS_CUDA(cudaStreamSynchronize(st));
@@ -191,10 +191,7 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
     // entries below 1e-18 ||K||_F are not rotated (they are far under the round-off of the updates)
     const double tiny = 1e-18 * std::sqrt(norm2);
     RS_CUDA(cudaMemcpyAsync(scal + 1, &tiny, sizeof(double), cudaMemcpyHostToDevice, st));
-    // one CTA per SM: G row-tile walkers per pair (and per (In, Out) set of the launch)
     const int tiles = npad / 64;
-    auto walkers = [&](int nz) { return std::max(1, std::min(tiles, P->num_sms / std::max(1, npairs * nz))); };
-    const dim3 grid2(npairs, walkers(2), 2), grid1(npairs, walkers(1), 1);
     double prev = -1.0;
     int sweep = 0;
     bool converged = norm2 == 0.0;
@@ -203,15 +200,14 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
         for (int r = 0; r < rounds; ++r) {
             const int2 *pr = P->eg_pairs.p + (size_t)r * npairs;
             rsdft::jacobi_subeig_kernel<<<npairs, 256, smem_sub, st>>>(Kp, npad, pr, P->eg_J.p, P->eig_inner, scal, r > 0 ? 1 : 0);
-            rsdft::ColUpdArgs u;
-            u.npad = npad; u.pairs = pr; u.Jbuf = P->eg_J.p;
-            u.In[0] = Kp; u.Out[0] = Tp; u.tr[0] = 1;            // Tp = (K Jt)^H = Jt^H K
-            u.In[1] = Va; u.Out[1] = Vb; u.tr[1] = 0;            // V  = V Jt
-            rsdft::jacobi_colupdate_kernel<<<grid2, 256, smem_upd, st>>>(u);
-            u.In[0] = Tp; u.Out[0] = Kp; u.tr[0] = 0;            // K  = Jt^H K Jt
-            rsdft::jacobi_colupdate_kernel<<<grid1, 256, smem_upd, st>>>(u);
+            rsdft::BlockUpdArgs u;
+            u.Kin = Kp; u.Kout = Tp; u.Vin = Va; u.Vout = Vb;
+            u.npad = npad; u.npairs = npairs; u.nk = npairs * (npairs + 1) / 2; u.tiles = tiles;
+            u.pairs = pr; u.Jbuf = P->eg_J.p;
+            rsdft::jacobi_block_update_kernel<<<u.nk + npairs * tiles, 256, smem_upd, st>>>(u);   // K = Jt^H K Jt and V = V Jt
+            std::swap(Kp, Tp);
             std::swap(Va, Vb);
-            P->last_launches += 3;
+            P->last_launches += 2;
         }
         rsdft::jacobi_offnorm_kernel<<<nred, 256, 0, st>>>(Kp, n, npad, scal + 8);
         rsdft::sum_partials_kernel<<<1, 32, 0, st>>>(scal + 8, nred, scal + 2);

@@ -13,8 +13,8 @@
 //                            blocks (round-robin tournament: nblk-1 rounds visit every pair once = one sweep);
 //                            jacobi_subeig_kernel diagonalises each pair's 64 x 64 Hermitian sub-matrix in shared
 //                            memory (parallel-ordered 2 x 2 rotations) and returns its unitary J; the update
-//                            K <- Jt^H K Jt, V <- V Jt (Jt = all pairs of the round) is three DMMA products
-//                            (jacobi_colupdate_kernel; the row update is a column update of the conjugate transpose).
+//                            K <- Jt^H K Jt, V <- V Jt (Jt = all pairs of the round) is ONE launch of DMMA products
+//                            over the 64 x 64 blocks (jacobi_block_update_kernel: J_a^H K_ab J_b per block).
 //                            Chosen over Householder tridiagonalisation + QL/D&C because every O(n^3) part is a
 //                            tensor-core product and the method is unconditionally accurate.
 #pragma once
@@ -396,66 +396,79 @@ __global__ void __launch_bounds__(256) jacobi_subeig_kernel(const double2 *Kp, i
     }
 }
 
-// Out[:, cols(p,q)] = In[:, cols(p,q)] * J_pair for every pair of the round (tr == 0), or the conjugate transpose
-// of that product stored at Out[cols(p,q), :] (tr == 1).  In, Out: npad x npad, Out != In.  Up to two independent
-// (In, Out, tr) sets per launch (blockIdx.z): the V update rides along with the first K update.
-// CTA (pair, g, z) keeps the pair's J (64 x 64) resident in shared memory and walks the 64-row tiles g, g + G, ...;
-// the next tile arrives by cp.async while the current one is multiplied: 8 warps, each 32 rows x 16 columns
-// (4 x 2 DMMA tiles), K = 64.
-struct ColUpdArgs {
-    const double2 *In[2];
-    double2 *Out[2];
-    int32_t tr[2];
-    int32_t npad;
+// The whole update of one Jacobi round in ONE launch.  With Jt = the block-diagonal of the round's pair rotations,
+// block (a, b) of K <- Jt^H K Jt (rows of pair a, columns of pair b, 64 x 64) is J_a^H K_ab J_b: it needs only the old
+// block and two J.  K is Hermitian, so only the blocks a <= b are formed and the others are written as their conjugate
+// transposes (the new K is Hermitian to the last bit off the diagonal blocks); V <- V Jt rides along as one product per
+// (pair, 64-row tile).  Items [0, nk) with nk = npairs (npairs + 1) / 2 are the K blocks (two products, the first
+// result T = K_ab J_b goes back to shared memory as the B operand of the second), items [nk, nk + npairs * tiles)
+// are the V tiles.  8 warps, each 32 rows x 16 columns (4 x 2 DMMA tiles), K = 64; operands K-major with pitch 68.
+struct BlockUpdArgs {
+    const double2 *Kin;
+    double2 *Kout;
+    const double2 *Vin;
+    double2 *Vout;
+    int32_t npad, npairs, nk, tiles;
     const int2 *pairs;
     const double2 *Jbuf;
 };
 
-__global__ void __launch_bounds__(256, 1) jacobi_colupdate_kernel(ColUpdArgs a)
+__global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArgs a)
 {
-    constexpr int D = 2 * EIG_JB, TM = 64, P = D + 4;
+    constexpr int D = 2 * EIG_JB, P = D + 4;
     extern __shared__ __align__(16) unsigned char eig_smem_raw[];
-    double2 *Bs = reinterpret_cast<double2 *>(eig_smem_raw);  // [D][P]      Bs[n*P + k] = J[k][n]
-    double2 *As0 = Bs + D * P;                                 // [2][TM][P]  As[m*P + k]
+    double2 *S0 = reinterpret_cast<double2 *>(eig_smem_raw);  // [D][P] A operand (K_ab or a V tile), then T^T
+    double2 *S1 = S0 + D * P;                                  // [D][P] S1[n*P + k] = J_b[k][n]
+    double2 *S2 = S1 + D * P;                                  // [D][P] S2[i*P + r] = J_a[r][i]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wm = warp >> 2, wn = warp & 3;
     const int g = lane >> 2, t = lane & 3;
-    const int z = blockIdx.z;
-    const double2 *In = a.In[z];
-    double2 *Out = a.Out[z];
-    const int tr = a.tr[z], npad = a.npad;
-    const int2 pq = a.pairs[blockIdx.x];
-    auto gcol = [&](int c) { return c < EIG_JB ? pq.x * EIG_JB + c : pq.y * EIG_JB + c - EIG_JB; };
-    const double2 *J = a.Jbuf + (int64_t)blockIdx.x * D * D;
-    for (int e = tid; e < D * D; e += 256) {
-        const int k = e % D, n = e / D;
-        cp_async16(Bs + n * P + k, J + e);
+    const int npad = a.npad;
+    const int item = blockIdx.x;
+    const bool kitem = item < a.nk;
+    int ia, ib, r0 = 0;
+    if (kitem) {
+        ib = (int)((sqrt(8.0 * item + 1.0) - 1.0) * 0.5);
+        while ((ib + 1) * (ib + 2) / 2 <= item) ++ib;
+        while (ib * (ib + 1) / 2 > item) --ib;
+        ia = item - ib * (ib + 1) / 2;
+    } else {
+        const int v = item - a.nk;
+        ia = ib = v / a.tiles;
+        r0 = (v - ia * a.tiles) * D;
     }
-    const int ntiles = npad / TM;
-    auto issue = [&](int buf, int rt) {
-        double2 *As = As0 + buf * TM * P;
-        const int r0 = rt * TM;
-        for (int e = tid; e < TM * D; e += 256) {
-            const int m = e % TM, k = e / TM;
-            cp_async16(As + m * P + k, In + (int64_t)gcol(k) * npad + r0 + m);
+    const int2 pa = a.pairs[ia], pb = a.pairs[ib];
+    auto idx = [&](int2 pq, int c) { return c < EIG_JB ? pq.x * EIG_JB + c : pq.y * EIG_JB + c - EIG_JB; };
+    // operand loads: S0[m*P + k] = In[row(m) + col_b(k)*npad]; S1 = J_b; S2 = J_a (K items only)
+    {
+        const double2 *In = kitem ? a.Kin : a.Vin;
+        for (int e = tid; e < D * D; e += 256) {
+            const int m = e % D, k = e / D;
+            const int row = kitem ? idx(pa, m) : r0 + m;
+            cp_async16(S0 + m * P + k, In + (int64_t)idx(pb, k) * npad + row);
         }
-    };
-    int rt = blockIdx.y;
-    if (rt < ntiles) issue(0, rt);
-    cp_async_commit();
-    int buf = 0;
-    for (; rt < ntiles; rt += gridDim.y, buf ^= 1) {
-        if (rt + (int)gridDim.y < ntiles) issue(buf ^ 1, rt + gridDim.y);
+        const double2 *Jb = a.Jbuf + (int64_t)ib * D * D;
+        for (int e = tid; e < D * D; e += 256) cp_async16(S1 + (e / D) * P + (e % D), Jb + e);
+        if (kitem) {
+            const double2 *Ja = a.Jbuf + (int64_t)ia * D * D;
+            for (int e = tid; e < D * D; e += 256) cp_async16(S2 + (e / D) * P + (e % D), Ja + e);
+        }
         cp_async_commit();
-        cp_async_wait<1>();
+        cp_async_wait<0>();
         __syncthreads();
-        double cre[4][2][2], cim[4][2][2];
+    }
+    double cre[4][2][2], cim[4][2][2];
+    auto zero = [&]() {
 #pragma unroll
         for (int x = 0; x < 4; ++x)
 #pragma unroll
             for (int y = 0; y < 2; ++y) { cre[x][y][0] = cre[x][y][1] = cim[x][y][0] = cim[x][y][1] = 0.0; }
-        const double2 *Ap = As0 + buf * TM * P + (wm * 32 + g) * P + t;
-        const double2 *Bp = Bs + (wn * 16 + g) * P + t;
+    };
+    // first product: C[m][n] = sum_k S0[m][k] * J_b[k][n]
+    zero();
+    {
+        const double2 *Ap = S0 + (wm * 32 + g) * P + t;
+        const double2 *Bp = S1 + (wn * 16 + g) * P + t;
 #pragma unroll 4
         for (int kk = 0; kk < D; kk += 4) {
             double br[2], bi[2];
@@ -477,7 +490,8 @@ __global__ void __launch_bounds__(256, 1) jacobi_colupdate_kernel(ColUpdArgs a)
                 }
             }
         }
-        const int r0 = rt * TM;
+    }
+    if (!kitem) {
 #pragma unroll
         for (int x = 0; x < 4; ++x)
 #pragma unroll
@@ -485,13 +499,60 @@ __global__ void __launch_bounds__(256, 1) jacobi_colupdate_kernel(ColUpdArgs a)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int row = r0 + wm * 32 + x * 8 + g;
-                    const int col = gcol(wn * 16 + y * 8 + 2 * t + e);
-                    if (tr) Out[(int64_t)row * npad + col] = make_double2(cre[x][y][e], -cim[x][y][e]);
-                    else Out[(int64_t)col * npad + row] = make_double2(cre[x][y][e], cim[x][y][e]);
+                    const int col = idx(pb, wn * 16 + y * 8 + 2 * t + e);
+                    a.Vout[(int64_t)col * npad + row] = make_double2(cre[x][y][e], cim[x][y][e]);
                 }
-        __syncthreads();                  // the buffer just read is the target of the next prefetch
+        return;
     }
-    cp_async_wait<0>();
+    __syncthreads();                                   // every warp has finished reading S0
+#pragma unroll
+    for (int x = 0; x < 4; ++x)
+#pragma unroll
+        for (int y = 0; y < 2; ++y)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int m = wm * 32 + x * 8 + g, n = wn * 16 + y * 8 + 2 * t + e;
+                S0[n * P + m] = make_double2(cre[x][y][e], cim[x][y][e]);          // T^T: B operand of the second product
+            }
+    __syncthreads();
+    // second product: C[i][j] = sum_r conj(J_a[r][i]) * T[r][j]
+    zero();
+    {
+        const double2 *Ap = S2 + (wm * 32 + g) * P + t;
+        const double2 *Bp = S0 + (wn * 16 + g) * P + t;
+#pragma unroll 4
+        for (int kk = 0; kk < D; kk += 4) {
+            double br[2], bi[2];
+#pragma unroll
+            for (int y = 0; y < 2; ++y) { const double2 v = Bp[y * 8 * P + kk]; br[y] = v.x; bi[y] = v.y; }
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                const double2 v = Ap[x * 8 * P + kk];
+                const double ar = v.x, ai = v.y, nai = -v.y;
+#pragma unroll
+                for (int y = 0; y < 2; ++y) {
+                    eig_dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
+                    eig_dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
+                }
+#pragma unroll
+                for (int y = 0; y < 2; ++y) {
+                    eig_dmma884(cre[x][y][0], cre[x][y][1], ai, bi[y]);
+                    eig_dmma884(cim[x][y][0], cim[x][y][1], nai, br[y]);
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int x = 0; x < 4; ++x)
+#pragma unroll
+        for (int y = 0; y < 2; ++y)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int row = idx(pa, wm * 32 + x * 8 + g);
+                const int col = idx(pb, wn * 16 + y * 8 + 2 * t + e);
+                a.Kout[(int64_t)col * npad + row] = make_double2(cre[x][y][e], cim[x][y][e]);
+                if (ia != ib) a.Kout[(int64_t)row * npad + col] = make_double2(cre[x][y][e], -cim[x][y][e]);
+            }
 }
 
 // Eigenvalues = real diagonal of the converged Kp; rank them ascending (ties by index), lambda[rank] = d for
