@@ -231,12 +231,17 @@ def max_over_ranks_value(x, world, device):
     return float(t.item())
 
 
-def gram_flops(n, ng, tile=96):
-    """(algorithmic, executed) flops of one rsdft_subspace_gram launch: H in full + S upper triangle; the executed
-    count includes the padding of the last 96-column tile and the full diagonal tiles of S."""
-    alg = 8.0 * ng * (n * n + n * (n + 1) / 2.0)
+GRAM_FLOPS_PER_CMAC = 6.0      # the kernel forms a complex multiply-add from 3 real MMAs (3M / Gauss form): 6 real flops, not 8
+GRAM_TILE = 48
+
+
+def gram_flops(n, ng, tile=GRAM_TILE):
+    """(algorithmic, executed) REAL flops of one rsdft_subspace_gram launch: H in full + S upper triangle, 6 real flops per
+    complex multiply-add (3M form; the conventional count is 8/6 of it); the executed count includes the padding of the
+    last 48-column tile and the full diagonal tiles of S."""
+    alg = GRAM_FLOPS_PER_CMAC * ng * (n * n + n * (n + 1) / 2.0)
     tm = (n + tile - 1) // tile
-    return alg, 8.0 * ng * tile * tile * (tm * tm + tm * (tm + 1) // 2)
+    return alg, GRAM_FLOPS_PER_CMAC * ng * tile * tile * (tm * tm + tm * (tm + 1) // 2)
 
 
 def free_all():
@@ -308,6 +313,7 @@ def time_block_step(rsdft, wl, torch, cfg_id, steps, warmup, sampler, peaks, hbm
     row = dict(workload=workload_name(cfg_id), steps=steps, warmup=warmup, ms_per_step=total_ms / steps, value=n * ng / (total_ms / steps * 1e-3),
                ms_apply_h=1e3 * t_apply, ms_gram=1e3 * t_gram, hx_pts_per_s=n * ng / t_apply,
                gram_tflops_executed=exe / t_gram / 1e12, gram_tflops_algorithmic=alg / t_gram / 1e12,
+               gram_tflops_conventional=alg * 8.0 / GRAM_FLOPS_PER_CMAC / t_gram / 1e12,
                roofline_gram_frac=(alg / t_gram / 1e12 / peaks["dmma_tflops"]) if peaks else None,
                roofline_apply_h_frac=bpp * ng * n / t_apply / 1e9 / hbm_peak, apply_h_model_bytes_per_point=bpp,
                apply_h_floor_frac=32.0 * ng * n / t_apply / 1e9 / hbm_peak,
@@ -390,7 +396,8 @@ def gemm_shape_rows(rsdft, wl, torch, sampler, peaks):
         del Y, HY
         free_all()
     return dict(rows=rows, clocks=sampler.window(m0) if sampler else None,
-                note="gram: [S|H] = Y^H [Y|HY], flops 8*K*(N^2 + N(N+1)/2) algorithmic (executed counts the 96-column tile padding); "
+                note="gram: [S|H] = Y^H [Y|HY], real flops 6*K*(N^2 + N(N+1)/2) algorithmic in the kernel's 3M form (executed counts the 48-column tile padding; "
+                     "the conventional 8-flop count is 4/3 of it); "
                      "rotate: Out[K x N/3] = Y[K x N] C, flops 8*K*N*m")
 
 
@@ -623,7 +630,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel: gram_dmma_kernel (timed region = the rsdft_subspace_gram call:
     # one gram_dmma_kernel launch + one gram_reduce_kernel launch of ~0.1 % of its duration)
     flops_alg, flops_exec = gram_flops(n, ng)
-    roofline = dict(bound="tensor", kernel="gram_dmma_kernel (FP64 DMMA.8x8x4)", achieved=flops_alg / t_gram / 1e12,
+    roofline = dict(bound="tensor", kernel="gram_dmma_kernel (FP64 DMMA.8x8x4, 3M complex product)", achieved=flops_alg / t_gram / 1e12,
                     peak=peaks["dmma_tflops"], unit="TFLOP/s", frac=flops_alg / t_gram / 1e12 / peaks["dmma_tflops"],
                     traffic=None,
                     traffic_source="not measured in this run (ncu cannot run inside the bench); the committed `ncu --set full` capture of this launch "
@@ -633,7 +640,11 @@ def run_ours(args):
                                 "(MEASURED_PEAKS.json has no FP64 entry; bf16 %.1f TF x nominal 40/2250 = %.1f TF for context)" % (
                                     (mp or {}).get("bf16_tflops", float("nan")), (mp or {}).get("bf16_tflops", float("nan")) * 40 / 2250),
                     flops_per_launch=flops_alg, executed_flops_per_launch=flops_exec, executed_tflops=flops_exec / t_gram / 1e12,
-                    ms_per_launch=1e3 * t_gram)
+                    ms_per_launch=1e3 * t_gram,
+                    flops_definition="REAL flops the method needs in the kernel's 3M complex product (3 real MMAs = 6 flops per complex multiply-add, "
+                                     "DESIGN.md 6.3): 6*Ng*(n^2 + n(n+1)/2) for H_sub in full + the upper triangle of S_sub; frac is the tensor-pipe view",
+                    conventional_8flop_tflops=flops_alg * 8.0 / GRAM_FLOPS_PER_CMAC / t_gram / 1e12,
+                    conventional_8flop_frac=flops_alg * 8.0 / GRAM_FLOPS_PER_CMAC / t_gram / 1e12 / peaks["dmma_tflops"])
     bpp = row["apply_h_model_bytes_per_point"]
     apply_roof = dict(bound="hbm", kernels="project/combine/fft3_fwd_zy/fft3_x/fft3_inv_yz/scatter (rsdft_apply_h)", achieved=bpp * ng * n / t_apply / 1e9,
                       peak=hbm_peak, peak_source="MEASURED_PEAKS.json hbm_gbs" if mp else "fallback 6650",
@@ -653,10 +664,11 @@ def run_ours(args):
                                               ncol_per_apply_call=row["ncol_per_apply_call"], apply_batch_cols=row["apply_batch_cols"], apply_streams=args.streams or 3,
                                               apply_fft_path={1: "persistent pipeline kernel (TMA tiles, L2-resident k-space)", 2: "three kernels per batch, TMA-staged x kernel"}.get(args.pipeline if args.pipeline >= 0 else 2, "three kernels per batch"), replicas=world),
                 hx_pts_per_s=n * ng / t_apply, gram_tflops=flops_exec / t_gram / 1e12,
-                gram_tflops_note="executed FP64 flops / t (H_sub in full + upper tiles of S_sub, incl. tile padding); "
-                                 "algorithmic (8*Ng*(n^2+n(n+1)/2)) = %.2f TF/s is roofline.achieved; the dense-equivalent 2*8*n^2*Ng count of SURVEY 8(d) "
-                                 "would read %.2f TF/s and is NOT work done (the lower triangle of S_sub is mirrored)" % (
-                                     flops_alg / t_gram / 1e12, 16.0 * n * n * ng / t_gram / 1e12),
+                gram_tflops_note="executed real FP64 flops / t (3M complex product: 6 flops per complex multiply-add; H_sub in full + upper tiles of "
+                                 "S_sub, incl. tile padding); algorithmic (6*Ng*(n^2+n(n+1)/2)) = %.2f TF/s is roofline.achieved; in the conventional 8-flop "
+                                 "count the same launch reads %.2f TF/s (roofline.conventional_8flop_tflops, above the DMMA peak because a quarter of the "
+                                 "multiplies is never executed); the dense-equivalent 2*8*n^2*Ng count of SURVEY 8(d) would read %.2f TF/s and is NOT work done" % (
+                                     flops_alg / t_gram / 1e12, flops_alg * 8.0 / GRAM_FLOPS_PER_CMAC / t_gram / 1e12, 16.0 * n * n * ng / t_gram / 1e12),
                 ms_apply_h=1e3 * t_apply, ms_gram=1e3 * t_gram, roofline=roofline, roofline_apply_h=apply_roof,
                 gram_hermitian_mode=dict(ms_gram=1e3 * t_gram_hu, ms_per_step=1e3 * (t_apply + t_gram_hu),
                                          value=world * n * ng / (t_apply + t_gram_hu), max_rel_diff_vs_full=dHu,

@@ -177,7 +177,7 @@ int rsdft_plan_set_eig_mode(rsdft_plan_t *plan, int32_t reduction, int32_t inner
 int rsdft_subspace_eig_stats(const rsdft_plan_t *plan, double *out8);
 
 /* One whole block step with HOST buffers (the end-to-end entry point): copies Y (host, pinned
- * recommended) to the device in panels of 96 columns; each panel goes through rsdft_apply_h as soon as
+ * recommended) to the device in panels of 96 columns (two Gram tile widths); each panel goes through rsdft_apply_h as soon as
  * it has arrived and then every [S|H] tile that has become computable is contracted, so both H Y and the
  * Gram matrices overlap the rest of the upload.  Copies H_sub, S_sub (and HY if HY_host != NULL) back to
  * the host and synchronises with the host before returning.  Results equal rsdft_apply_h +
@@ -216,7 +216,7 @@ int rsdft_plan_set_streams(rsdft_plan_t *plan, int32_t nstreams);
 int rsdft_plan_set_pipeline(rsdft_plan_t *plan, int32_t mode);
 
 /* Gram mode.  0 (default): H_sub = Y^H (HY) is contracted in full, as the definition reads (and as the
- * paper's ZGEMM does), so it is Hermitian only to round-off.  1: only the upper 96-column
+ * paper's ZGEMM does), so it is Hermitian only to round-off.  1: only the upper 48-column
  * tiles of H_sub are contracted and the rest is their conjugate mirror with a real diagonal, like S_sub
  * (H is Hermitian, hence so is Y^H H Y in exact arithmetic; Hermitian eigen-solvers read one triangle
  * anyway): 30 % fewer flops, H_sub exactly Hermitian, equal to mode 0 within round-off.

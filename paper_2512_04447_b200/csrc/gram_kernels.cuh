@@ -8,7 +8,14 @@
 // fragment layout of m8n8k4, so tiles are staged into shared memory as plain interleaved
 // complex128 with cp.async and read back as one 128-bit LDS per fragment (re, im).
 //
-// One complex product = 4 real MMAs:  re += Ar*Br;  re += Ai*Bi;  im += Ar*Bi;  im += (-Ai)*Br.
+// One complex product conj(a) b = 3 real MMAs (the "3M" / Gauss form, as in BLAS ZGEMM3M):
+//     K1 += (Ar - Ai) * Br,   K2 += Ar * (Bi - Br),   K3 += (-Ai) * (Br + Bi);     re = K1 - K3,   im = K1 + K2
+// -- a quarter fewer tensor-core instructions than the 4-product form (re += Ar*Br + Ai*Bi, im += Ar*Bi - Ai*Br, kept as
+// M3 = false for comparison) at the price of a third accumulator set, which is why the tile is 48 x 48 and not 96 x 96
+// (a 96 x 96 tile with three accumulator sets would take 84 % of the SM's register file).  The operand combinations are
+// formed once per fragment load.  The sums K1..K3 are up to twice as large as re / im, so the normwise error bound grows
+// by a small constant (measured against the long-double oracle: see DESIGN.md); it is not componentwise stable, which
+// the normwise parity bar of north_star does not ask for.
 //
 // Work decomposition: a unit = (K-slab, output tile).  Tiles are TM x TN complex; S_sub only
 // needs its upper-triangular tiles (it is exactly Hermitian), H_sub is computed in full.
@@ -56,8 +63,8 @@ struct GramCfg {
 
 // BULK: the operand rows of a stage (KC consecutive grid points of one column = 256 contiguous bytes) arrive by ONE
 // TMA bulk copy each (cp.async.bulk + mbarrier, SASS UBLKCP) instead of KC per-thread 16-byte cp.async (LDGSTS).
-template <int WGM, int WGN, int FA, int FB, int KC, int STAGES, bool BULK = false>
-__global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES, bool BULK = false, bool M3 = true, int MINB = 1>
+__global__ void __launch_bounds__(WGM *WGN * 32, MINB) gram_dmma_kernel(GramArgs a)
 {
     using Cfg = GramCfg<WGM, WGN, FA, FB, KC, STAGES>;
     constexpr int TM = Cfg::TM, TN = Cfg::TN, PITCH = Cfg::PITCH, NT = Cfg::THREADS;
@@ -125,11 +132,15 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
             bulk_g2s(sm + (size_t)stage * Cfg::STAGE_ELEMS + tid * PITCH, my_src + (int64_t)chunk * KC, KC * sizeof(double2), &full_bar[stage]);
     };
 
-    double cre[FA][FB][2], cim[FA][FB][2];
+    double cre[FA][FB][2], cim[FA][FB][2];       // 4M: re, im;  3M: K1, K2
+    double ck3[M3 ? FA : 1][M3 ? FB : 1][2];     // 3M: K3
 #pragma unroll
     for (int x = 0; x < FA; ++x)
 #pragma unroll
-        for (int y = 0; y < FB; ++y) { cre[x][y][0] = cre[x][y][1] = 0.0; cim[x][y][0] = cim[x][y][1] = 0.0; }
+        for (int y = 0; y < FB; ++y) {
+            cre[x][y][0] = cre[x][y][1] = 0.0; cim[x][y][0] = cim[x][y][1] = 0.0;
+            if (M3) ck3[x][y][0] = ck3[x][y][1] = 0.0;
+        }
 
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
@@ -150,22 +161,39 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
         const double2 *Bs = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + (TM + wn * FB * 8 + g) * PITCH + t;
 #pragma unroll
         for (int kk = 0; kk < KC; kk += 4) {
-            double br[FB], bi[FB];
+            if (M3) {
+                double b0[FB], b1[FB], b2[FB];
 #pragma unroll
-            for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PITCH + kk]; br[y] = v.x; bi[y] = v.y; }
+                for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PITCH + kk]; b0[y] = v.x; b1[y] = v.y - v.x; b2[y] = v.x + v.y; }
 #pragma unroll
-            for (int x = 0; x < FA; ++x) {
-                const double2 v = As[x * 8 * PITCH + kk];
-                const double ar = v.x, ai = v.y, nai = -v.y;
+                for (int x = 0; x < FA; ++x) {
+                    const double2 v = As[x * 8 * PITCH + kk];
+                    const double a0 = v.x - v.y, a1 = v.x, a2 = -v.y;
 #pragma unroll
-                for (int y = 0; y < FB; ++y) {
-                    dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
-                    dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
+                    for (int y = 0; y < FB; ++y) {
+                        dmma884(cre[x][y][0], cre[x][y][1], a0, b0[y]);
+                        dmma884(cim[x][y][0], cim[x][y][1], a1, b1[y]);
+                        dmma884(ck3[x][y][0], ck3[x][y][1], a2, b2[y]);
+                    }
                 }
+            } else {
+                double br[FB], bi[FB];
 #pragma unroll
-                for (int y = 0; y < FB; ++y) {
-                    dmma884(cre[x][y][0], cre[x][y][1], ai, bi[y]);
-                    dmma884(cim[x][y][0], cim[x][y][1], nai, br[y]);
+                for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PITCH + kk]; br[y] = v.x; bi[y] = v.y; }
+#pragma unroll
+                for (int x = 0; x < FA; ++x) {
+                    const double2 v = As[x * 8 * PITCH + kk];
+                    const double ar = v.x, ai = v.y, nai = -v.y;
+#pragma unroll
+                    for (int y = 0; y < FB; ++y) {
+                        dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
+                        dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
+                    }
+#pragma unroll
+                    for (int y = 0; y < FB; ++y) {
+                        dmma884(cre[x][y][0], cre[x][y][1], ai, bi[y]);
+                        dmma884(cim[x][y][0], cim[x][y][1], nai, br[y]);
+                    }
                 }
             }
         }
@@ -182,7 +210,7 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) gram_dmma_kernel(GramArgs a)
             for (int e = 0; e < 2; ++e) {
                 const int ii = (wm * FA + x) * 8 + g;
                 const int jj = (wn * FB + y) * 8 + 2 * t + e;
-                W[jj * TM + ii] = make_double2(cre[x][y][e], cim[x][y][e]);
+                W[jj * TM + ii] = M3 ? make_double2(cre[x][y][e] - ck3[x][y][e], cre[x][y][e] + cim[x][y][e]) : make_double2(cre[x][y][e], cim[x][y][e]);
             }
 }
 

@@ -920,13 +920,16 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
     return RSDFT_OK;
 }
 
-// Gram configuration: 96 x 96 complex tile, 8 warps (2 x 4), each 48 x 24 = 6 x 3 DMMA tiles
-#ifndef RSDFT_GRAM_WGM      // warps along M, warps along N, fragments per warp along M, along N, stages
-#define RSDFT_GRAM_WGM 2
-#define RSDFT_GRAM_WGN 4
-#define RSDFT_GRAM_FA 6
+// Gram configuration: 48 x 48 complex tile, 4 warps (2 x 2), each 24 x 24 = 3 x 3 DMMA tiles with three accumulator sets (3M
+// complex product, gram_kernels.cuh), two CTAs per SM
+#ifndef RSDFT_GRAM_WGM      // warps along M, warps along N, fragments per warp along M, along N, stages, 3M product, CTAs per SM
+#define RSDFT_GRAM_WGM 2    // (the 4-product form of round 1: 2, 4, 6, 3, 3, false, 1 -- a 96 x 96 tile)
+#define RSDFT_GRAM_WGN 2
+#define RSDFT_GRAM_FA 3
 #define RSDFT_GRAM_FB 3
 #define RSDFT_GRAM_STAGES 3
+#define RSDFT_GRAM_M3 true
+#define RSDFT_GRAM_MINB 2
 #endif
 #define RSDFT_GRAM_SHAPE RSDFT_GRAM_WGM, RSDFT_GRAM_WGN, RSDFT_GRAM_FA, RSDFT_GRAM_FB, 16, RSDFT_GRAM_STAGES
 using GCfg = GramCfg<RSDFT_GRAM_SHAPE>;
@@ -950,18 +953,18 @@ int choose_kslabs(int64_t ntiles, int64_t nchunks, int sms)
 // One launch of the Gram kernels over `ntiles` tiles of a device tile list (any subset of the
 // [S|H] tiles): split-K contraction into the tile-indexed workspace, then the fixed-order reduce.
 int gram_launch(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2 *HY, int64_t ldhy, double2 *H, double2 *S,
-                int lds, const GramTile *dtiles, int ntiles, cudaStream_t st)
+                int lds, const GramTile *dtiles, int ntiles, cudaStream_t st, int ks_fixed = 0)
 {
     if (ntiles == 0) return RSDFT_OK;
     const int64_t nchunks = P->ng / GRAM_KC;
-    const int ks = choose_kslabs(ntiles, nchunks, P->num_sms);
+    const int ks = ks_fixed > 0 ? ks_fixed : choose_kslabs(ntiles, nchunks, P->num_sms * RSDFT_GRAM_MINB);
     if ((size_t)ks * ntiles * GCfg::TM * GCfg::TN > P->gram_work.n)
         return fail(RSDFT_ALLOC, "gram_launch: workspace smaller than the launch needs (internal)");
     GramArgs a;
     a.Y = Y; a.HY = HY; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = ntiles; a.kslabs = ks;
     a.nchunks = nchunks; a.tiles = dtiles; a.work = P->gram_work.p;
     // operand staging: TMA bulk copies (gram_bulk, rsdft_plan_set_gram_mode) or per-thread cp.async
-    auto kern = P->gram_bulk ? gram_dmma_kernel<RSDFT_GRAM_SHAPE, true> : gram_dmma_kernel<RSDFT_GRAM_SHAPE, false>;
+    auto kern = P->gram_bulk ? gram_dmma_kernel<RSDFT_GRAM_SHAPE, true, RSDFT_GRAM_M3, RSDFT_GRAM_MINB> : gram_dmma_kernel<RSDFT_GRAM_SHAPE, false, RSDFT_GRAM_M3, RSDFT_GRAM_MINB>;
     // the attribute is per device/context: set it on every launch (cheap), never cache it per thread
     RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
     kern<<<ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);
@@ -978,7 +981,7 @@ int gram_launch(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const doubl
 size_t gram_work_need(const rsdft_plan *P, int ntiles)
 {
     if (ntiles == 0) return 0;
-    return (size_t)choose_kslabs(ntiles, P->ng / GRAM_KC, P->num_sms) * ntiles * GCfg::TM * GCfg::TN;
+    return (size_t)choose_kslabs(ntiles, P->ng / GRAM_KC, P->num_sms * RSDFT_GRAM_MINB) * ntiles * GCfg::TM * GCfg::TN;
 }
 
 // the whole [S|H]: H tiles row-major, then the upper S tiles
@@ -1000,12 +1003,16 @@ int gram_impl(rsdft_plan *P, int n, const double2 *Y, int64_t ldy, const double2
         P->gram_ntiles = (int)tiles.size();
         P->gram_tiles_n = key;
     }
-    RS_CUDA(P->gram_work.ensure(gram_work_need(P, P->gram_ntiles)));
-    return gram_launch(P, n, Y, ldy, HY, ldhy, H, S, lds, P->gram_tiles.p, P->gram_ntiles, st);
+    // the K split is the one of the full [S|H] launch whichever outputs are asked for, so that S_sub (or H_sub) alone
+    // comes out bit for bit as it does together with the other matrix
+    const int full = tm * tm + tm * (tm + 1) / 2;              // (also the same in both Gram modes)
+    const int ks = choose_kslabs(full, P->ng / GRAM_KC, P->num_sms * RSDFT_GRAM_MINB);
+    RS_CUDA(P->gram_work.ensure((size_t)ks * P->gram_ntiles * GCfg::TM * GCfg::TN));
+    return gram_launch(P, n, Y, ldy, HY, ldhy, H, S, lds, P->gram_tiles.p, P->gram_ntiles, st, ks);
 }
 
 // tile list ordered by column panel (panel t = tile column t): panel t holds every [S|H] tile that
-// becomes computable when columns [0, 96(t+1)) are on the device: H(i<=t, t), H(t, j<t), S(i<=t, t).
+// becomes computable when columns [0, TM(t+1)) are on the device (TM = the Gram tile width): H(i<=t, t), H(t, j<t), S(i<=t, t).
 int gram_panel_lists(rsdft_plan *P, int n, cudaStream_t st)
 {
     const int key = 2 * n + P->gram_h_upper;
@@ -1192,7 +1199,7 @@ int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ld
                         void *H_sub, void *S_sub, int32_t lds, void *stream)
 {
     if (!plan || !Y) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: null argument");
-    if (n <= 0 || n > 32767 * 96) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: n out of range");
+    if (n <= 0 || n > 32767 * GCfg::TM) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: n out of range");
     if (!H_sub && !S_sub) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: both outputs null");
     if (H_sub && !HY) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: H_sub requested without HY");
     if (ldy < plan->ng || (H_sub && ldhy < plan->ng)) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram: ld < Ng");
@@ -1262,12 +1269,14 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
         RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev_vloc, 0));
         P->vloc_pending = false;
     }
-    // Column panels of one Gram tile width (96 columns): the H2D copy of panel k+1 overlaps apply_h and
+    // Column panels of two Gram tile widths (96 columns; apply_h keeps efficient batches): the H2D copy of panel k+1 overlaps apply_h and
     // the Gram tiles of panel k.  After panel t has been through H, every [S|H] tile that involves only
-    // columns < 96(t+1) and touches panel t is contracted, so the Gram (the long part of the step) runs
+    // columns < TM(t+1) and touches panel t is contracted, so the Gram (the long part of the step) runs
     // while the rest of Y is still crossing PCIe instead of after the last byte has arrived.
-    const int chunk = GCfg::TM;
+    constexpr int TPP = 2;                                     // Gram tile columns per upload panel
+    const int chunk = TPP * GCfg::TM;
     const int nchunk = (n + chunk - 1) / chunk;
+    const int ntcol = (n + GCfg::TM - 1) / GCfg::TM;          // tile columns = entries of gram_panel_off - 1
     while ((int)P->ev.size() < 2 * nchunk) {
         cudaEvent_t e;
         RS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -1276,7 +1285,12 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     int rc = gram_panel_lists(P, n, P->s_comp);
     if (rc != RSDFT_OK) return rc;
     size_t need = 0;
-    for (int k = 0; k < nchunk; ++k) need = std::max(need, gram_work_need(P, P->gram_panel_off[k + 1] - P->gram_panel_off[k]));
+    auto tiles_of = [&](int k, int &first) {                   // tile-list range that becomes computable with upload panel k
+        const int t0 = std::min(k * TPP, ntcol), t1 = std::min((k + 1) * TPP, ntcol);
+        first = P->gram_panel_off[t0];
+        return P->gram_panel_off[t1] - first;
+    };
+    for (int k = 0; k < nchunk; ++k) { int f; need = std::max(need, gram_work_need(P, tiles_of(k, f))); }
     RS_CUDA(P->gram_work.ensure(need));
     double2 *Hd = P->hostHS.p, *Sd = P->hostHS.p + (size_t)n * n;
     P->last_launches = 0;
@@ -1296,8 +1310,9 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
             RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], P->s_comp));
             launches += P->last_launches;
             P->last_launches = 0;
-            r = gram_launch(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->gram_panel_tiles.p + P->gram_panel_off[k],
-                            P->gram_panel_off[k + 1] - P->gram_panel_off[k], P->s_comp);
+            int first = 0;
+            const int nt = tiles_of(k, first);
+            r = gram_launch(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->gram_panel_tiles.p + first, nt, P->s_comp);
             if (r != RSDFT_OK) return r;
             launches += P->last_launches;
             P->last_launches = 0;
