@@ -634,8 +634,8 @@ def run_ours(args):
                     peak=peaks["dmma_tflops"], unit="TFLOP/s", frac=flops_alg / t_gram / 1e12 / peaks["dmma_tflops"],
                     traffic=None,
                     traffic_source="not measured in this run (ncu cannot run inside the bench); the committed `ncu --set full` capture of this launch "
-                                   "(profiles/r2_ncu_full_config2.md) read 203.7 GB of DRAM per launch = 5.0x the 40.8 GB operand floor (2*n*Ng*16 B), "
-                                   "i.e. 310 GB/s on a compute-bound kernel",
+                                   "(profiles/r2_ncu_full_config2.md) read 632.7 GB of DRAM per launch = 15.5x the 40.8 GB operand floor (2*n*Ng*16 B), "
+                                   "i.e. 1.23 TB/s = 15 % of the DRAM peak on a compute-bound kernel (48 x 48 tiles re-read the panels through L2)",
                     peak_source="libpeakprobe DMMA.8x8x4 register loop on this GPU, 150 launches back to back, clock record in peaks_probe.clocks "
                                 "(MEASURED_PEAKS.json has no FP64 entry; bf16 %.1f TF x nominal 40/2250 = %.1f TF for context)" % (
                                     (mp or {}).get("bf16_tflops", float("nan")), (mp or {}).get("bf16_tflops", float("nan")) * 40 / 2250),
