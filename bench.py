@@ -390,7 +390,8 @@ def gemm_shape_rows(rsdft, wl, torch, sampler, peaks):
             tr = timed(torch, lambda: rsdft.rsdft_subspace_rotate(plan, Y[:N], Cm, Out), 2)
             rows.append(dict(N=N, K=K, K_over_N=K / N, gram_ms=1e3 * t, gram_tflops_algorithmic=alg / t / 1e12,
                              gram_tflops_executed=exe / t / 1e12, gram_frac_of_dmma_peak=alg / t / 1e12 / peaks["dmma_tflops"],
-                             rotate_m=mrot, rotate_ms=1e3 * tr, rotate_tflops=8.0 * K * N * mrot / tr / 1e12))
+                             rotate_m=mrot, rotate_ms=1e3 * tr, rotate_tflops=GRAM_FLOPS_PER_CMAC * K * N * mrot / tr / 1e12,
+                             rotate_tflops_conventional=8.0 * K * N * mrot / tr / 1e12))
             del Hs, Ss, Cm, Out
         plan.close()
         del Y, HY
@@ -398,7 +399,7 @@ def gemm_shape_rows(rsdft, wl, torch, sampler, peaks):
     return dict(rows=rows, clocks=sampler.window(m0) if sampler else None,
                 note="gram: [S|H] = Y^H [Y|HY], real flops 6*K*(N^2 + N(N+1)/2) algorithmic in the kernel's 3M form (executed counts the 48-column tile padding; "
                      "the conventional 8-flop count is 4/3 of it); "
-                     "rotate: Out[K x N/3] = Y[K x N] C, flops 8*K*N*m")
+                     "rotate: Out[K x N/3] = Y[K x N] C, real flops 6*K*N*m (3M form; conventional 8*K*N*m beside it)")
 
 
 def library_yardstick(torch, st):
@@ -529,15 +530,17 @@ def run_ours(args):
     if Cm is not None and "error" not in eig and free_b > (3 * m * ng * 16 + (4 << 30)):
         Xn = torch.empty((m, ng), dtype=torch.complex128, device="cuda")
         t_rot = timed(torch, lambda: rsdft.rsdft_subspace_rotate(plan, Y, Cm, Xn), 3)
-        fl = 8.0 * ng * n * m
+        fl = GRAM_FLOPS_PER_CMAC * ng * n * m          # real flops of the 3M complex product (6 per complex multiply-add)
         rot = dict(ms=1e3 * t_rot, tflops=fl / t_rot / 1e12, frac_of_dmma_peak=fl / t_rot / 1e12 / peaks["dmma_tflops"],
-                   shape="Out[Ng x %d] = Y[Ng x %d] C[%d x %d]" % (m, n, n, m), note="rsdft_subspace_rotate, one call (X' = Y C_X); flops 8*Ng*n*m")
+                   conventional_8flop_tflops=fl * 8.0 / GRAM_FLOPS_PER_CMAC / t_rot / 1e12,
+                   shape="Out[Ng x %d] = Y[Ng x %d] C[%d x %d]" % (m, n, n, m), note="rsdft_subspace_rotate, one call (X' = Y C_X); real flops 6*Ng*n*m (3M product)")
         HXn = torch.empty_like(Xn); R = torch.empty_like(Xn)
         t_rot2 = timed(torch, lambda: rsdft.rsdft_subspace_rotate2(plan, Y, HY, Cm, lam, Xn, HXn, R), 2)
         rnorm = float(R.abs().max() / HXn.abs().max())
         rot2 = dict(ms=1e3 * t_rot2, tflops=2 * fl / t_rot2 / 1e12, frac_of_dmma_peak=2 * fl / t_rot2 / 1e12 / peaks["dmma_tflops"],
+                    conventional_8flop_tflops=2 * fl * 8.0 / GRAM_FLOPS_PER_CMAC / t_rot2 / 1e12,
                     max_abs_R_over_max_abs_HXnew=rnorm, algorithmic_bytes=(2 * n + 3 * m) * ng * 16,
-                    note="rsdft_subspace_rotate2: X' = Y C, HX' = HY C, R = HX' - X' Lambda in one pass with the Ritz pairs of next1_eig; flops 16*Ng*n*m "
+                    note="rsdft_subspace_rotate2: X' = Y C, HX' = HY C, R = HX' - X' Lambda in one pass with the Ritz pairs of next1_eig; real flops 12*Ng*n*m (3M product) "
                          "(the block is random, so the residual is large: one Rayleigh-Ritz step of an unconverged LOBPCG)")
         del Xn, HXn, R
 

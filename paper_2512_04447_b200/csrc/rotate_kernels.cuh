@@ -44,8 +44,10 @@ struct RotateCfg {
     static constexpr size_t SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(double2);
 };
 
-template <int WGM, int WGN, int FA, int FB, int KC, int STAGES>
-__global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate_dmma_kernel(RotateArgs a)
+// M3: the complex product a b from three real MMAs (K1 += (Ar + Ai) Br, K2 += Ar (Bi - Br), K3 += Ai (Br + Bi);
+// re = K1 - K3, im = K1 + K2), as in gram_kernels.cuh; needs a third accumulator set, hence smaller tiles.
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES, bool M3 = false, int MINB = 1>
+__global__ void __launch_bounds__(WGM *WGN * 32, MINB) rotate_dmma_kernel(RotateArgs a)
 {
     using Cfg = RotateCfg<WGM, WGN, FA, FB, KC, STAGES>;
     constexpr int TM = Cfg::TM, TN = Cfg::TN, PA = Cfg::PA, PB = Cfg::PB, NT = Cfg::THREADS;
@@ -83,11 +85,15 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate_dmma_kernel(RotateArg
         }
     };
 
-    double cre[FA][FB][2], cim[FA][FB][2];
+    double cre[FA][FB][2], cim[FA][FB][2];       // 4M: re, im;  3M: K1, K2
+    double ck3[M3 ? FA : 1][M3 ? FB : 1][2];     // 3M: K3
 #pragma unroll
     for (int x = 0; x < FA; ++x)
 #pragma unroll
-        for (int y = 0; y < FB; ++y) { cre[x][y][0] = cre[x][y][1] = 0.0; cim[x][y][0] = cim[x][y][1] = 0.0; }
+        for (int y = 0; y < FB; ++y) {
+            cre[x][y][0] = cre[x][y][1] = 0.0; cim[x][y][0] = cim[x][y][1] = 0.0;
+            if (M3) ck3[x][y][0] = ck3[x][y][1] = 0.0;
+        }
 
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
@@ -105,7 +111,24 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate_dmma_kernel(RotateArg
         const double2 *As = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + t * PA + wm * FA * 8 + g;
         const double2 *Bs = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + KC * PA + (wn * FB * 8 + g) * PB + t;
 #pragma unroll
-        for (int kk = 0; kk < KC; kk += 4) {
+        for (int kk = 0; M3 && kk < KC; kk += 4) {
+            double b0[FB], b1[FB], b2[FB];
+#pragma unroll
+            for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PB + kk]; b0[y] = v.x; b1[y] = v.y - v.x; b2[y] = v.x + v.y; }
+#pragma unroll
+            for (int x = 0; x < FA; ++x) {
+                const double2 v = As[kk * PA + x * 8];
+                const double a0 = v.x + v.y;
+#pragma unroll
+                for (int y = 0; y < FB; ++y) {
+                    rot_dmma884(cre[x][y][0], cre[x][y][1], a0, b0[y]);
+                    rot_dmma884(cim[x][y][0], cim[x][y][1], v.x, b1[y]);
+                    rot_dmma884(ck3[x][y][0], ck3[x][y][1], v.y, b2[y]);
+                }
+            }
+        }
+#pragma unroll
+        for (int kk = 0; !M3 && kk < KC; kk += 4) {
             double br[FB], bi[FB];
 #pragma unroll
             for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PB + kk]; br[y] = v.x; bi[y] = v.y; }
@@ -138,7 +161,8 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate_dmma_kernel(RotateArg
             for (int e = 0; e < 2; ++e) {
                 const int64_t r = r0 + (wm * FA + x) * 8 + g;
                 const int j = j0 + (wn * FB + y) * 8 + 2 * t + e;
-                if (r < a.ng && j < a.m) a.Out[(int64_t)j * a.ldo + r] = make_double2(cre[x][y][e], cim[x][y][e]);
+                if (r < a.ng && j < a.m)
+                    a.Out[(int64_t)j * a.ldo + r] = M3 ? make_double2(cre[x][y][e] - ck3[x][y][e], cre[x][y][e] + cim[x][y][e]) : make_double2(cre[x][y][e], cim[x][y][e]);
             }
 }
 
@@ -166,8 +190,8 @@ struct Rotate2Cfg {
     static constexpr size_t SMEM = (size_t)STAGES * STAGE_ELEMS * sizeof(double2);
 };
 
-template <int WGM, int WGN, int FA, int FB, int KC, int STAGES>
-__global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate2_dmma_kernel(Rotate2Args a)
+template <int WGM, int WGN, int FA, int FB, int KC, int STAGES, bool M3 = false, int MINB = 1>
+__global__ void __launch_bounds__(WGM *WGN * 32, MINB) rotate2_dmma_kernel(Rotate2Args a)
 {
     using Cfg = Rotate2Cfg<WGM, WGN, FA, FB, KC, STAGES>;
     constexpr int TM = Cfg::TM, TN = Cfg::TN, PA = Cfg::PA, PB = Cfg::PB, NT = Cfg::THREADS;
@@ -209,13 +233,17 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate2_dmma_kernel(Rotate2A
         }
     };
 
-    double xre[FA][FB][2], xim[FA][FB][2], hre[FA][FB][2], him[FA][FB][2];
+    double xre[FA][FB][2], xim[FA][FB][2], hre[FA][FB][2], him[FA][FB][2];      // 4M: re, im;  3M: K1, K2
+    double xk3[M3 ? FA : 1][M3 ? FB : 1][2], hk3[M3 ? FA : 1][M3 ? FB : 1][2];  // 3M: K3
 #pragma unroll
     for (int x = 0; x < FA; ++x)
 #pragma unroll
         for (int y = 0; y < FB; ++y)
 #pragma unroll
-            for (int e = 0; e < 2; ++e) { xre[x][y][e] = xim[x][y][e] = hre[x][y][e] = him[x][y][e] = 0.0; }
+            for (int e = 0; e < 2; ++e) {
+                xre[x][y][e] = xim[x][y][e] = hre[x][y][e] = him[x][y][e] = 0.0;
+                if (M3) xk3[x][y][e] = hk3[x][y][e] = 0.0;
+            }
 
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
@@ -234,7 +262,28 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate2_dmma_kernel(Rotate2A
         const double2 *Hs = As + KC * PA;
         const double2 *Bs = sm + (size_t)(ch % STAGES) * Cfg::STAGE_ELEMS + 2 * KC * PA + (wn * FB * 8 + g) * PB + t;
 #pragma unroll
-        for (int kk = 0; kk < KC; kk += 4) {
+        for (int kk = 0; M3 && kk < KC; kk += 4) {
+            double b0[FB], b1[FB], b2[FB];
+#pragma unroll
+            for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PB + kk]; b0[y] = v.x; b1[y] = v.y - v.x; b2[y] = v.x + v.y; }
+#pragma unroll
+            for (int x = 0; x < FA; ++x) {
+                const double2 v = As[kk * PA + x * 8];
+                const double2 w = Hs[kk * PA + x * 8];
+                const double v0 = v.x + v.y, w0 = w.x + w.y;
+#pragma unroll
+                for (int y = 0; y < FB; ++y) {
+                    rot_dmma884(xre[x][y][0], xre[x][y][1], v0, b0[y]);
+                    rot_dmma884(xim[x][y][0], xim[x][y][1], v.x, b1[y]);
+                    rot_dmma884(xk3[x][y][0], xk3[x][y][1], v.y, b2[y]);
+                    rot_dmma884(hre[x][y][0], hre[x][y][1], w0, b0[y]);
+                    rot_dmma884(him[x][y][0], him[x][y][1], w.x, b1[y]);
+                    rot_dmma884(hk3[x][y][0], hk3[x][y][1], w.y, b2[y]);
+                }
+            }
+        }
+#pragma unroll
+        for (int kk = 0; !M3 && kk < KC; kk += 4) {
             double br[FB], bi[FB];
 #pragma unroll
             for (int y = 0; y < FB; ++y) { const double2 v = Bs[y * 8 * PB + kk]; br[y] = v.x; bi[y] = v.y; }
@@ -273,9 +322,11 @@ __global__ void __launch_bounds__(WGM *WGN * 32, 1) rotate2_dmma_kernel(Rotate2A
             for (int x = 0; x < FA; ++x) {
                 const int64_t r = r0 + (wm * FA + x) * 8 + g;
                 if (r >= a.ng) continue;
-                if (a.X) a.X[(int64_t)j * a.ldx + r] = make_double2(xre[x][y][e], xim[x][y][e]);
-                if (a.HX) a.HX[(int64_t)j * a.ldhx + r] = make_double2(hre[x][y][e], him[x][y][e]);
-                if (a.R) a.R[(int64_t)j * a.ldr + r] = make_double2(fma(-lam, xre[x][y][e], hre[x][y][e]), fma(-lam, xim[x][y][e], him[x][y][e]));
+                const double xr = M3 ? xre[x][y][e] - xk3[x][y][e] : xre[x][y][e], xi = M3 ? xre[x][y][e] + xim[x][y][e] : xim[x][y][e];
+                const double hr = M3 ? hre[x][y][e] - hk3[x][y][e] : hre[x][y][e], hi = M3 ? hre[x][y][e] + him[x][y][e] : him[x][y][e];
+                if (a.X) a.X[(int64_t)j * a.ldx + r] = make_double2(xr, xi);
+                if (a.HX) a.HX[(int64_t)j * a.ldhx + r] = make_double2(hr, hi);
+                if (a.R) a.R[(int64_t)j * a.ldr + r] = make_double2(fma(-lam, xr, hr), fma(-lam, xi, hi));
             }
         }
 }

@@ -1227,22 +1227,23 @@ int rsdft_subspace_rotate(rsdft_plan_t *plan, int32_t n, int32_t m, const void *
     RotateArgs a;
     a.Y = (const double2 *)Y; a.C = (const double2 *)Cmat; a.Out = (double2 *)Out;
     a.ldy = ldy; a.ldo = ldo; a.ng = plan->ng; a.n = n; a.m = m; a.ldc = ldc;
-    // output tile 96 x 96 or 64 x 128 (rows x columns), whichever pads m less (m = 480 -> 96, m = 512 -> 128)
-    const bool wide = ((m + 127) / 128) * 128 < ((m + 95) / 96) * 96;
-    using R96 = RotateCfg<2, 4, 6, 3, 16, 3>;
-    using R128 = RotateCfg<2, 4, 4, 4, 16, 3>;
-    const int tm = wide ? R128::TM : R96::TM, tn = wide ? R128::TN : R96::TN;
+    // 3M complex product (rotate_kernels.cuh): output tile 48 x 48 or 48 x 64 (rows x columns), whichever pads m less
+    // (m = 480 -> 48, m = 512 -> 64), four warps with three accumulator sets, two CTAs per SM
+    const bool wide = ((m + 63) / 64) * 64 < ((m + 47) / 48) * 48;
+    using R48 = RotateCfg<2, 2, 3, 3, 16, 3>;
+    using R64 = RotateCfg<2, 2, 3, 4, 16, 3>;
+    const int tm = wide ? R64::TM : R48::TM, tn = wide ? R64::TN : R48::TN;
     a.jtiles = (m + tn - 1) / tn;
     const int64_t units = ((plan->ng + tm - 1) / tm) * a.jtiles;
     if (units > 0x7fffffffll) return fail(RSDFT_UNSUPPORTED, "rsdft_subspace_rotate: too many tiles for one launch");
     if (wide) {
-        auto kern = rotate_dmma_kernel<2, 4, 4, 4, 16, 3>;
-        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R128::SMEM));
-        kern<<<(unsigned)units, R128::THREADS, R128::SMEM, (cudaStream_t)stream>>>(a);
+        auto kern = rotate_dmma_kernel<2, 2, 3, 4, 16, 3, true, 2>;
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R64::SMEM));
+        kern<<<(unsigned)units, R64::THREADS, R64::SMEM, (cudaStream_t)stream>>>(a);
     } else {
-        auto kern = rotate_dmma_kernel<2, 4, 6, 3, 16, 3>;
-        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R96::SMEM));
-        kern<<<(unsigned)units, R96::THREADS, R96::SMEM, (cudaStream_t)stream>>>(a);
+        auto kern = rotate_dmma_kernel<2, 2, 3, 3, 16, 3, true, 2>;
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R48::SMEM));
+        kern<<<(unsigned)units, R48::THREADS, R48::SMEM, (cudaStream_t)stream>>>(a);
     }
     plan->last_launches = 1;
     RS_CUDA(cudaGetLastError());
@@ -1370,22 +1371,17 @@ int rsdft_subspace_rotate2(rsdft_plan_t *plan, int32_t n, int32_t m, const void 
     a.Y = (const double2 *)Y; a.HY = (const double2 *)HY; a.C = (const double2 *)Cmat; a.lambda = lambda;
     a.X = (double2 *)Xout; a.HX = (double2 *)HXout; a.R = (double2 *)R;
     a.ldy = ldy; a.ldhy = ldhy; a.ldx = ldx; a.ldhx = ldhx; a.ldr = ldr; a.ng = ng; a.n = n; a.m = m; a.ldc = ldc;
-    // 96 x 48 or 96 x 64 output tile (rows x columns), whichever pads m less (m = 480 -> 48, m = 512 -> 64)
-    using R48 = Rotate2Cfg<4, 2, 3, 3, 16, 3>;
-    using R64 = Rotate2Cfg<4, 2, 3, 4, 16, 3>;
-    const bool wide = ((m + 63) / 64) * 64 <= ((m + 47) / 48) * 48;
-    const int tm = R48::TM, tn = wide ? R64::TN : R48::TN;
+    // 3M complex product with six accumulator sets (X': K1..K3, HX': K1..K3): 48 x 32 output tile (rows x columns), four
+    // warps of 3 x 2 fragments, two CTAs per SM
+    using R32 = Rotate2Cfg<2, 2, 3, 2, 16, 3>;
+    const int tm = R32::TM, tn = R32::TN;
     a.jtiles = (m + tn - 1) / tn;
     const int64_t units = ((ng + tm - 1) / tm) * a.jtiles;
     if (units > 0x7fffffffll) return fail(RSDFT_UNSUPPORTED, "rsdft_subspace_rotate2: too many tiles for one launch");
-    if (wide) {
-        auto kern = rotate2_dmma_kernel<4, 2, 3, 4, 16, 3>;
-        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R64::SMEM));
-        kern<<<(unsigned)units, R64::THREADS, R64::SMEM, (cudaStream_t)stream>>>(a);
-    } else {
-        auto kern = rotate2_dmma_kernel<4, 2, 3, 3, 16, 3>;
-        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R48::SMEM));
-        kern<<<(unsigned)units, R48::THREADS, R48::SMEM, (cudaStream_t)stream>>>(a);
+    {
+        auto kern = rotate2_dmma_kernel<2, 2, 3, 2, 16, 3, true, 2>;
+        RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)R32::SMEM));
+        kern<<<(unsigned)units, R32::THREADS, R32::SMEM, (cudaStream_t)stream>>>(a);
     }
     plan->last_launches = 1;
     RS_CUDA(cudaGetLastError());
