@@ -2,8 +2,9 @@
 //   Out[r, j] = sum_c Y[r, c] * C[c, j],   r < Ng grid points, c < n subspace columns, j < m new columns,
 // e.g. X' = Y C_X, HX' = HY C_X, P' = [W, P] C_P.  Tall-skinny times small: M = Ng (~10^6), K = n (~1500),
 // N = m (~500).  Like the Gram contraction it is a dense FP64 product, so it runs on the FP64 tensor pipe
-// (mma.sync.m8n8k4.f64, the only native FP64 MMA shape of sm_100a), one complex product = 4 real MMAs:
-//   re += Ar*Br;  re += (-Ai)*Bi;  im += Ar*Bi;  im += Ai*Br.
+// (mma.sync.m8n8k4.f64, the only native FP64 MMA shape of sm_100a).  One complex product is 4 real MMAs in the plain
+// form (M3 = false):  re += Ar*Br;  re += (-Ai)*Bi;  im += Ar*Bi;  im += Ai*Br,  and 3 in the 3M form the launchers use
+// (M3 = true, see the kernel templates below).
 //
 // Operand layouts.  A = Y is "M-major" in memory (a column of Y is contiguous in r), the opposite of what the
 // row fragment of m8n8k4 wants, so a stage holds A as [k][r] with pitch TM+2 complex (pitch % 8 == 2: the 8
