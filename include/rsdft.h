@@ -125,6 +125,28 @@ int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ld
                         const void *HY, int64_t ldhy, void *H_sub, void *S_sub, int32_t lds,
                         void *stream);
 
+/* rsdft_subspace_gram for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the same contraction (PAPER.md:19 task (2)), the same
+ * arguments, layouts and output rules as rsdft_subspace_gram (the plan's Gram mode is honoured, its staging knob
+ * is not), but the split-K partial tiles and the tile list live in a file-scope `static __device__` scratch of
+ * RSDFT_GRAM_STATIC_WORK_BYTES + 12.1 KiB inside the library instead of plan-owned workspace.  The call
+ * performs no cudaMalloc / cudaFree and calls no allocating library routine, never synchronises, and launches
+ * three kernels on `stream`.  Every GPU that loads the library holds the scratch until exit.
+ * Limit: n <= RSDFT_GRAM_STATIC_MAX_N (any Ng); a larger n returns RSDFT_UNSUPPORTED with a message and launches
+ * nothing.  When the K split rsdft_subspace_gram would take does not fit the scratch it is cut down, so results
+ * equal rsdft_subspace_gram's bit for bit where the split fits and to round-off (1e-12 normwise) otherwise.
+ * The scratch is ONE array per device, shared by every call and every plan on that device, and keeps the last
+ * call's contents: nothing in it needs to start at zero (each call overwrites all it reads), but two calls
+ * that overlap on the GPU (different streams without an ordering between them, or concurrent graph branches)
+ * race on it -- the caller must order them.  The first call on a device resolves the scratch address
+ * (cudaGetSymbolAddress, which loads the module): make it outside stream capture.
+ * Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+#define RSDFT_GRAM_STATIC_MAX_N 1536
+#define RSDFT_GRAM_STATIC_WORK_BYTES 67108864 /* 64 MiB */
+int rsdft_subspace_gram_static(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ldy,
+                               const void *HY, int64_t ldhy, void *H_sub, void *S_sub, int32_t lds,
+                               void *stream);
+
 /* Rayleigh-Ritz update of LOBPCG (the step after the eigen-solve of the (H_sub, S_sub) pencil; Knyazev's
  * method as cited by PAPER.md:19,124):
  *   Out[r, j] = sum_{c < n} Y[r, c] * C[c, j],   j < m,   e.g. X' = Y C_X, HX' = HY C_X, P' = [W, P] C_P.

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1054,6 +1055,73 @@ bool overlaps(const void *a, size_t na, const void *b, size_t nb)
 }  // namespace
 
 // ------------------------------------------------------------------------------------------
+// rsdft_subspace_gram_static: the Gram contraction for callers that cannot allocate (CUDA graph capture, serving loops).
+// Its split-K partial tiles and its tile list live in the two file-scope arrays below instead of plan-owned cudaMalloc
+// buffers: RSDFT_GRAM_STATIC_WORK_BYTES (64 MiB) + 12.1 KiB of device memory on every GPU that loads the library, held
+// until exit.  Every call on a device shares them.  In host code the array names are host-side stand-ins, not device
+// addresses: gram_static_scratch() resolves them with cudaGetSymbolAddress once per device.
+constexpr int GRAM_STATIC_MAX_N = RSDFT_GRAM_STATIC_MAX_N;
+constexpr int GRAM_STATIC_MAX_TCOLS = (GRAM_STATIC_MAX_N + GCfg::TM - 1) / GCfg::TM;
+constexpr int GRAM_STATIC_MAX_TILES = GRAM_STATIC_MAX_TCOLS * GRAM_STATIC_MAX_TCOLS + GRAM_STATIC_MAX_TCOLS * (GRAM_STATIC_MAX_TCOLS + 1) / 2;
+constexpr size_t GRAM_STATIC_WORK_ELEMS = (size_t)RSDFT_GRAM_STATIC_WORK_BYTES / sizeof(double2);
+static_assert((size_t)GRAM_STATIC_MAX_TILES * GCfg::TM * GCfg::TN <= GRAM_STATIC_WORK_ELEMS,
+              "RSDFT_GRAM_STATIC_WORK_BYTES too small for RSDFT_GRAM_STATIC_MAX_N columns at one K slab");
+
+static __device__ __align__(256) double2 g_gram_static_work[GRAM_STATIC_WORK_ELEMS];        // [kslabs][ntiles][TN][TM]
+static __device__ __align__(256) rsdft::GramTile g_gram_static_tiles[GRAM_STATIC_MAX_TILES];
+
+// The tile list gram_impl builds on the host (H tiles row-major -- from the diagonal on in the Hermitian mode -- then the
+// upper S tiles), written on the device so that no upload buffer is needed.  tc = tile columns.
+__global__ void gram_static_tiles_kernel(int tc, int want_h, int want_s, int h_upper)
+{
+    const int upper = tc * (tc + 1) / 2;
+    const int nh = want_h ? (h_upper ? upper : tc * tc) : 0;
+    const int nt = nh + (want_s ? upper : 0);
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < nt; e += gridDim.x * blockDim.x) {
+        const bool is_h = e < nh;
+        int i, j;
+        if (is_h && !h_upper) { i = e / tc; j = e - i * tc; }
+        else {                                   // e-th pair (i <= j) in row-major order
+            int r = is_h ? e : e - nh;
+            i = 0;
+            while (r >= tc - i) { r -= tc - i; ++i; }
+            j = i + r;
+        }
+        rsdft::GramTile t;
+        t.ti = (int16_t)i; t.tj = (int16_t)j; t.mat = (int16_t)(is_h ? (h_upper ? 2 : 0) : 1); t.pad = 0;
+        g_gram_static_tiles[e] = t;              // device code names the array directly
+    }
+}
+
+namespace {
+
+struct GramStaticScratch { double2 *work; rsdft::GramTile *tiles; };
+
+// Device addresses of the two arrays for the CURRENT device (`dev`), resolved once per device.
+int gram_static_scratch(int dev, GramStaticScratch &out)
+{
+    constexpr int MAXDEV = 64;
+    static std::mutex mu;
+    static GramStaticScratch cache[MAXDEV];
+    static bool have[MAXDEV];
+    if (dev < 0 || dev >= MAXDEV) return fail(RSDFT_UNSUPPORTED, "rsdft_subspace_gram_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!have[dev]) {
+        GramStaticScratch s{nullptr, nullptr};
+        RS_CUDA(cudaGetSymbolAddress((void **)&s.work, g_gram_static_work));
+        RS_CUDA(cudaGetSymbolAddress((void **)&s.tiles, g_gram_static_tiles));
+        if (!s.work || !s.tiles || ((uintptr_t)s.work & 255))
+            return fail(RSDFT_CUDA, "rsdft_subspace_gram_static: cudaGetSymbolAddress returned an unusable address");
+        cache[dev] = s;
+        have[dev] = true;
+    }
+    out = cache[dev];
+    return RSDFT_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
 // C ABI
 
 extern "C" {
@@ -1210,6 +1278,50 @@ int rsdft_subspace_gram(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ld
     plan->last_launches = 0;
     return gram_impl(plan, n, (const double2 *)Y, ldy, H_sub ? (const double2 *)HY : nullptr, ldhy, (double2 *)H_sub,
                      (double2 *)S_sub, lds, (cudaStream_t)stream);
+}
+
+int rsdft_subspace_gram_static(rsdft_plan_t *plan, int32_t n, const void *Y, int64_t ldy, const void *HY, int64_t ldhy,
+                               void *H_sub, void *S_sub, int32_t lds, void *stream)
+{
+    if (!plan || !Y) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram_static: null argument");
+    if (n <= 0) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram_static: n out of range");
+    if (n > GRAM_STATIC_MAX_N)
+        return fail(RSDFT_UNSUPPORTED, "rsdft_subspace_gram_static: n = " + std::to_string(n) + " exceeds RSDFT_GRAM_STATIC_MAX_N = " +
+                                           std::to_string(GRAM_STATIC_MAX_N) + " (the static scratch of " +
+                                           std::to_string(RSDFT_GRAM_STATIC_WORK_BYTES >> 20) + " MiB holds no more); use rsdft_subspace_gram");
+    if (!H_sub && !S_sub) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram_static: both outputs null");
+    if (H_sub && !HY) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram_static: H_sub requested without HY");
+    if (ldy < plan->ng || (H_sub && ldhy < plan->ng)) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram_static: ld < Ng");
+    if (lds < n) return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram_static: lds < n");
+    if (((uintptr_t)Y | (uintptr_t)HY | (uintptr_t)H_sub | (uintptr_t)S_sub) & 15)
+        return fail(RSDFT_INVALID_ARG, "rsdft_subspace_gram_static: pointers must be 16-byte aligned");
+    if (int rc = check_device(plan, "rsdft_subspace_gram_static")) return rc;
+    GramStaticScratch sc;
+    if (int rc = gram_static_scratch(plan->device, sc)) return rc;
+
+    const cudaStream_t st = (cudaStream_t)stream;
+    const int tc = (n + GCfg::TM - 1) / GCfg::TM;
+    const int upper = tc * (tc + 1) / 2;
+    const int ntiles = (H_sub ? (plan->gram_h_upper ? upper : tc * tc) : 0) + (S_sub ? upper : 0);
+    // the K split rsdft_subspace_gram takes (so that the two agree bit for bit), cut down to what the scratch holds
+    const int64_t nchunks = plan->ng / GRAM_KC;
+    int ks = choose_kslabs(tc * tc + upper, nchunks, plan->num_sms * RSDFT_GRAM_MINB);
+    ks = (int)std::max<size_t>(1, std::min<size_t>((size_t)ks, GRAM_STATIC_WORK_ELEMS / ((size_t)ntiles * GCfg::TM * GCfg::TN)));
+
+    gram_static_tiles_kernel<<<(ntiles + 255) / 256, 256, 0, st>>>(tc, H_sub != nullptr, S_sub != nullptr, plan->gram_h_upper);
+    GramArgs a;
+    a.Y = (const double2 *)Y; a.HY = H_sub ? (const double2 *)HY : nullptr; a.ldy = ldy; a.ldhy = ldhy; a.n = n; a.ntiles = ntiles;
+    a.kslabs = ks; a.nchunks = nchunks; a.tiles = sc.tiles; a.work = sc.work;
+    auto kern = gram_dmma_kernel<RSDFT_GRAM_SHAPE, false, RSDFT_GRAM_M3, RSDFT_GRAM_MINB>;
+    RS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GCfg::SMEM));
+    kern<<<ntiles * ks, GCfg::THREADS, GCfg::SMEM, st>>>(a);      // every (slab, tile) of the scratch it reads later is written here in full:
+    GramReduceArgs r;                                             // nothing has to start at zero
+    r.work = sc.work; r.tiles = sc.tiles; r.H = (double2 *)H_sub; r.S = (double2 *)S_sub; r.n = n; r.lds = lds; r.kslabs = ks; r.ntiles = ntiles;
+    r.tm = GCfg::TM; r.tn = GCfg::TN;
+    gram_reduce_kernel<<<ntiles, 256, 0, st>>>(r);
+    plan->last_launches = 3;
+    RS_CUDA(cudaGetLastError());
+    return RSDFT_OK;
 }
 
 int rsdft_subspace_rotate(rsdft_plan_t *plan, int32_t n, int32_t m, const void *Y, int64_t ldy, const void *Cmat, int32_t ldc,

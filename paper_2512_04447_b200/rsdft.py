@@ -5,7 +5,7 @@ if the library is missing, or it reports an error, the call raises.  torch is us
 memory and streams only (torch tensors' data_ptr() / torch.cuda.current_stream()).
 
 Function names follow the C ABI: rsdft_plan_create, rsdft_plan_set_vloc, rsdft_apply_h,
-rsdft_subspace_gram, rsdft_subspace_rotate, rsdft_subspace_rotate2, rsdft_subspace_eig, rsdft_subspace_eig_get,
+rsdft_subspace_gram, rsdft_subspace_gram_static, rsdft_subspace_rotate, rsdft_subspace_rotate2, rsdft_subspace_eig, rsdft_subspace_eig_get,
 rsdft_plan_set_eig_mode, rsdft_subspace_eig_stats, rsdft_block_step_host, rsdft_plan_release_workspace, rsdft_plan_info,
 rsdft_plan_set_batch, rsdft_plan_set_streams, rsdft_plan_set_gram_mode, rsdft_plan_destroy, rsdft_last_error.  Orbital blocks are torch complex128 tensors of shape
 [ncol, ld] (row c = column c of the paper's block, contiguous in the grid index)."""
@@ -17,7 +17,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librsdft.so")
 
-SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram", "rsdft_subspace_rotate",
+SYMBOLS = ["rsdft_plan_create", "rsdft_plan_set_vloc", "rsdft_apply_h", "rsdft_subspace_gram", "rsdft_subspace_gram_static",
+           "rsdft_subspace_rotate",
            "rsdft_subspace_rotate2", "rsdft_subspace_eig", "rsdft_subspace_eig_get", "rsdft_plan_set_eig_mode",
            "rsdft_subspace_eig_stats", "rsdft_plan_release_workspace", "rsdft_plan_set_pipeline", "rsdft_plan_set_gram_staging",
            "rsdft_block_step_host", "rsdft_plan_info", "rsdft_plan_set_batch", "rsdft_plan_set_streams", "rsdft_plan_set_gram_mode", "rsdft_plan_destroy",
@@ -75,6 +76,7 @@ def load():
     lib.rsdft_plan_set_vloc.argtypes = [vp, vp, vp]
     lib.rsdft_apply_h.argtypes = [vp, i32, vp, i64, vp, i64, vp]
     lib.rsdft_subspace_gram.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32, vp]
+    lib.rsdft_subspace_gram_static.argtypes = [vp, i32, vp, i64, vp, i64, vp, vp, i32, vp]
     lib.rsdft_subspace_rotate.argtypes = [vp, i32, i32, vp, i64, vp, i32, vp, i64, vp]
     lib.rsdft_subspace_rotate2.argtypes = [vp, i32, i32, vp, i64, vp, i64, vp, i32, vp, vp, i64, vp, i64, vp, i64, vp]
     lib.rsdft_subspace_eig.argtypes = [vp, i32, vp, vp, i32, i32, vp, vp, i32, vp]
@@ -248,6 +250,35 @@ def rsdft_apply_h(plan, X, HX, stream=None):
     _check(load().rsdft_apply_h(plan.handle, ncol, C.c_void_p(X.data_ptr()), ldx, C.c_void_p(HX.data_ptr()), ldhx,
                                 _stream(stream)))
     return HX
+
+
+RSDFT_GRAM_STATIC_MAX_N = 1536
+
+
+def rsdft_subspace_gram_static(plan, Y, HY, H_sub, S_sub, stream=None):
+    """rsdft_subspace_gram through the entry point that allocates nothing: the caller passes the outputs ([n, lds >= n]
+    complex128 CUDA tensors, column-major as rsdft_subspace_gram's; None skips one, HY may be None without H_sub); the
+    scratch is the library's static device array; n <= RSDFT_GRAM_STATIC_MAX_N.  -> (H_sub, S_sub)."""
+    if H_sub is None and S_sub is None:
+        raise ValueError("rsdft_subspace_gram_static: the caller passes at least one output")
+    n, ldy = _block(Y, "Y", plan)
+    ldhy = ldy
+    if H_sub is not None:
+        n2, ldhy = _block(HY, "HY", plan)
+        if n2 != n:
+            raise ValueError("Y and HY disagree on n")
+    lds = None
+    for t, name in ((H_sub, "H_sub"), (S_sub, "S_sub")):
+        if t is not None:
+            ld = _matrix(t, name, n, n)
+            if lds is not None and ld != lds:
+                raise ValueError("H_sub and S_sub must share one leading dimension")
+            lds = ld
+    _check(load().rsdft_subspace_gram_static(plan.handle, n, C.c_void_p(Y.data_ptr()), ldy,
+                                             C.c_void_p(HY.data_ptr()) if H_sub is not None else None, ldhy,
+                                             C.c_void_p(H_sub.data_ptr()) if H_sub is not None else None,
+                                             C.c_void_p(S_sub.data_ptr()) if S_sub is not None else None, lds, _stream(stream)))
+    return H_sub, S_sub
 
 
 def rsdft_subspace_gram(plan, Y, HY, H_sub=None, S_sub=None, stream=None, want_h=True, want_s=True):
