@@ -1410,6 +1410,11 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     int64_t launches = 0;
     // everything below is queued on the two plan-owned streams; on ANY error both are drained before the
     // call returns, so no copy or kernel of a failed call is still touching the caller's host buffers
+#ifdef RSDFT_LAB_TIMELINE      // lab builds only: per-panel event times on stderr
+    std::vector<cudaEvent_t> tl(3 * nchunk + 1);
+    for (auto &e : tl) cudaEventCreate(&e);
+    cudaEventRecord(tl[3 * nchunk], P->s_copy);
+#endif
     auto body = [&]() -> int {
         for (int k = 0; k < nchunk; ++k) {
             const int c0 = k * chunk, nc = std::min(chunk, n - c0);
@@ -1417,16 +1422,25 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
                                       (const char *)Y_host + (size_t)c0 * ldy * 16, (size_t)ldy * 16, (size_t)ng * 16, nc,
                                       cudaMemcpyHostToDevice, P->s_copy));
             RS_CUDA(cudaEventRecord(P->ev[2 * k], P->s_copy));
+#ifdef RSDFT_LAB_TIMELINE
+            cudaEventRecord(tl[3 * k], P->s_copy);
+#endif
             RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev[2 * k], 0));
             int r = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, P->s_comp);
             if (r != RSDFT_OK) return r;
             RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], P->s_comp));
+#ifdef RSDFT_LAB_TIMELINE
+            cudaEventRecord(tl[3 * k + 1], P->s_comp);
+#endif
             launches += P->last_launches;
             P->last_launches = 0;
             int first = 0;
             const int nt = tiles_of(k, first);
             r = gram_launch(P, n, P->hostY.p, ng, P->hostHY.p, ng, Hd, Sd, n, P->gram_panel_tiles.p + first, nt, P->s_comp);
             if (r != RSDFT_OK) return r;
+#ifdef RSDFT_LAB_TIMELINE
+            cudaEventRecord(tl[3 * k + 2], P->s_comp);
+#endif
             launches += P->last_launches;
             P->last_launches = 0;
         }
@@ -1446,6 +1460,15 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     };
     rc = body();
     const cudaError_t e1 = cudaStreamSynchronize(P->s_comp), e2 = cudaStreamSynchronize(P->s_copy);
+#ifdef RSDFT_LAB_TIMELINE
+    for (int k = 0; k < nchunk; ++k) {
+        float t[3];
+        for (int j = 0; j < 3; ++j) cudaEventElapsedTime(&t[j], tl[3 * nchunk], tl[3 * k + j]);
+        int f;
+        fprintf(stderr, "panel %2d: upload done %8.2f  apply_h done %8.2f  gram done %8.2f ms  (%d tiles)\n", k, t[0], t[1], t[2], tiles_of(k, f));
+    }
+    for (auto &e : tl) cudaEventDestroy(e);
+#endif
     if (rc != RSDFT_OK) return rc;
     RS_CUDA(e1);
     RS_CUDA(e2);
