@@ -44,8 +44,11 @@ struct SphereTables {
 };
 
 // scatter: CG complex values in flight per point.
+#ifndef RSDFT_NL_CG9
+#define RSDFT_NL_CG9 4
+#endif
 template <int NP> struct NlCols {
-    static constexpr int CGS = NP <= 4 ? 8 : (NP <= 9 ? 4 : 2);
+    static constexpr int CGS = NP <= 4 ? 8 : (NP <= 9 ? RSDFT_NL_CG9 : 2);
 };
 
 // Projection as a skinny FP64 tensor-core contraction with a gathered operand:
