@@ -192,34 +192,76 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
     const double tiny = 1e-18 * std::sqrt(norm2);
     RS_CUDA(cudaMemcpyAsync(scal + 1, &tiny, sizeof(double), cudaMemcpyHostToDevice, st));
     const int tiles = npad / 64;
+    // Two streams per round: `hi` carries the chain sub-problems -> K update -> next sub-problems (the 23 sub-problem
+    // CTAs are a latency chain on 23 SMs), `lo` carries V <- V Jt, which nothing needs before the end and which fills
+    // the other SMs meanwhile.  J is double-buffered by round parity; ev J[p] = J of that parity written, V[p] = read.
+    bool ovl = P->eig_overlap != 0;
+#ifdef RSDFT_LAB_N
+    if (const char *e = getenv("RSDFT_LAB_EIGOVL")) ovl = atoi(e) != 0;
+#endif
+    cudaStream_t hi = st, lo = st;
+    if (ovl) {
+        if (!P->eg_s_hi) {
+            int plo = 0, phi = 0;
+            RS_CUDA(cudaDeviceGetStreamPriorityRange(&plo, &phi));
+            RS_CUDA(cudaStreamCreateWithPriority(&P->eg_s_hi, cudaStreamNonBlocking, phi));
+            RS_CUDA(cudaStreamCreateWithPriority(&P->eg_s_lo, cudaStreamNonBlocking, plo));
+            for (auto &e : P->eg_sync) RS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        }
+        hi = P->eg_s_hi; lo = P->eg_s_lo;
+        RS_CUDA(cudaEventRecord(P->eg_sync[4], st));            // fork: both streams start behind the caller's stream
+        RS_CUDA(cudaStreamWaitEvent(hi, P->eg_sync[4], 0));
+        RS_CUDA(cudaStreamWaitEvent(lo, P->eg_sync[4], 0));
+    }
+    const size_t jsz = (size_t)npairs * D * D;
     double prev = -1.0;
     int sweep = 0;
+    int64_t gr = 0;                                             // rounds so far (parity picks the J buffer)
     bool converged = norm2 == 0.0;
     const int max_sweeps = 30;
     for (; sweep < max_sweeps && !converged; ++sweep) {
-        for (int r = 0; r < rounds; ++r) {
+        for (int r = 0; r < rounds; ++r, ++gr) {
+            const int par = ovl ? (int)(gr & 1) : 0;
+            double2 *Jb = P->eg_J.p + (size_t)par * jsz;
             const int2 *pr = P->eg_pairs.p + (size_t)r * npairs;
-            rsdft::jacobi_subeig_kernel<<<npairs, 256, smem_sub, st>>>(Kp, npad, pr, P->eg_J.p, P->eig_inner, scal, r > 0 ? 1 : 0);
+            if (ovl && gr >= 2) RS_CUDA(cudaStreamWaitEvent(hi, P->eg_sync[2 + par], 0));    // the V update two rounds back has read this J buffer
+            rsdft::jacobi_subeig_kernel<<<npairs, rsdft::EIG_SUB_NT, smem_sub, hi>>>(Kp, npad, pr, Jb, P->eig_inner, scal, r > 0 ? 1 : 0);
             rsdft::BlockUpdArgs u;
             u.Kin = Kp; u.Kout = Tp; u.Vin = Va; u.Vout = Vb;
             u.npad = npad; u.npairs = npairs; u.nk = npairs * (npairs + 1) / 2; u.tiles = tiles;
-            u.pairs = pr; u.Jbuf = P->eg_J.p;
-            rsdft::jacobi_block_update_kernel<<<u.nk + npairs * tiles, 256, smem_upd, st>>>(u);   // K = Jt^H K Jt and V = V Jt
+            u.pairs = pr; u.Jbuf = Jb; u.item0 = 0;
+            if (ovl) {
+                RS_CUDA(cudaEventRecord(P->eg_sync[par], hi));
+                rsdft::jacobi_block_update_kernel<<<u.nk, 256, smem_upd, hi>>>(u);                       // K = Jt^H K Jt
+                RS_CUDA(cudaStreamWaitEvent(lo, P->eg_sync[par], 0));
+                u.item0 = u.nk;
+                rsdft::jacobi_block_update_kernel<<<npairs * tiles, 256, smem_upd, lo>>>(u);             // V = V Jt
+                RS_CUDA(cudaEventRecord(P->eg_sync[2 + par], lo));
+                P->last_launches += 3;
+            } else {
+                rsdft::jacobi_block_update_kernel<<<u.nk + npairs * tiles, 256, smem_upd, st>>>(u);      // both in one launch
+                P->last_launches += 2;
+            }
             std::swap(Kp, Tp);
             std::swap(Va, Vb);
-            P->last_launches += 2;
         }
-        rsdft::jacobi_offnorm_kernel<<<nred, 256, 0, st>>>(Kp, n, npad, scal + 8);
-        rsdft::sum_partials_kernel<<<1, 32, 0, st>>>(scal + 8, nred, scal + 2);
+        rsdft::jacobi_offnorm_kernel<<<nred, 256, 0, hi>>>(Kp, n, npad, scal + 8);
+        rsdft::sum_partials_kernel<<<1, 32, 0, hi>>>(scal + 8, nred, scal + 2);
         P->last_launches += 2;
         RS_CUDA(cudaGetLastError());
-        RS_CUDA(cudaMemcpyAsync(host + 2, scal + 2, sizeof(double), cudaMemcpyDeviceToHost, st));
-        RS_CUDA(cudaStreamSynchronize(st));
+        RS_CUDA(cudaMemcpyAsync(host + 2, scal + 2, sizeof(double), cudaMemcpyDeviceToHost, hi));
+        RS_CUDA(cudaStreamSynchronize(hi));
         const double off = host[2];
         // converged: off(K) <= 1e-13 ||K||_F, or the round-off floor is reached (no further decrease below 1e-10)
         if (off <= 1e-26 * norm2) converged = true;
         else if (prev >= 0.0 && off > 0.25 * prev && off <= 1e-20 * norm2) converged = true;
         prev = off;
+    }
+    if (ovl) {                                                  // join: the caller's stream continues behind both
+        RS_CUDA(cudaEventRecord(P->eg_sync[5], lo));
+        RS_CUDA(cudaStreamWaitEvent(st, P->eg_sync[5], 0));
+        RS_CUDA(cudaEventRecord(P->eg_sync[5], hi));
+        RS_CUDA(cudaStreamWaitEvent(st, P->eg_sync[5], 0));
     }
     P->eig_stats[0] = sweep;
     P->eig_stats[5] = norm2 > 0.0 ? std::sqrt(prev < 0.0 ? 0.0 : prev / norm2) : 0.0;
@@ -242,7 +284,7 @@ static int eig_impl(rsdft_plan *P, int n, const double2 *H, const double2 *S, in
     RS_CUDA(P->eg_Z.ensure(nn));
     RS_CUDA(P->eg_Dinv.ensure((size_t)nblk * NB * NB));
     RS_CUDA(P->eg_Kp.ensure(np2)); RS_CUDA(P->eg_Tp.ensure(np2)); RS_CUDA(P->eg_V0.ensure(np2)); RS_CUDA(P->eg_V1.ensure(np2));
-    RS_CUDA(P->eg_J.ensure((size_t)(npad / D) * D * D));
+    RS_CUDA(P->eg_J.ensure((size_t)2 * (npad / D) * D * D));      // two buffers (round parity)
     RS_CUDA(P->eg_Zs.ensure((size_t)n * m));
     RS_CUDA(P->eg_scal.ensure(8 + 148));
     RS_CUDA(P->eg_info.ensure(1));

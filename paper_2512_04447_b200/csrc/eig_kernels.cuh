@@ -308,10 +308,18 @@ __global__ void __launch_bounds__(256) jacobi_offnorm_kernel(const double2 *Kp, 
 // over the nblk-1 rounds of a sweep every off-diagonal element is then annihilated exactly once (cyclic Jacobi in
 // a block round-robin ordering); the first round of each sweep runs with cross == 0 and also covers the pairs
 // inside the two diagonal blocks (63 steps).
-__global__ void __launch_bounds__(256) jacobi_subeig_kernel(const double2 *Kp, int npad, const int2 *pairs, double2 *Jbuf,
-                                                            int inner, const double *norm2, int cross)
+#ifndef RSDFT_EIG_SUB_NT
+#define RSDFT_EIG_SUB_NT 1024
+#endif
+constexpr int EIG_SUB_NT = RSDFT_EIG_SUB_NT;
+// A step is a latency chain (rotation parameters -> update -> next parameters) on one SM, so the CTA is as wide as it
+// gets: warp 0 computes the 32 rotations (reciprocal square roots instead of square roots and divisions), then every
+// thread applies them.  A <- J^H A J is done per 2 x 2 block (row pair k1, column pair k2: the column rotation of k2,
+// then the row rotation of k1, on the four elements in registers), so a step needs two barriers and one pass over A.
+__global__ void __launch_bounds__(EIG_SUB_NT) jacobi_subeig_kernel(const double2 *Kp, int npad, const int2 *pairs, double2 *Jbuf,
+                                                                   int inner, const double *norm2, int cross)
 {
-    constexpr int D = 2 * EIG_JB, P = D + 1;
+    constexpr int D = 2 * EIG_JB, P = D + 1, NT = EIG_SUB_NT;
     extern __shared__ __align__(16) unsigned char eig_smem_raw[];
     double2 *A = reinterpret_cast<double2 *>(eig_smem_raw);   // [D][P]
     double2 *V = A + D * P;
@@ -322,7 +330,7 @@ __global__ void __launch_bounds__(256) jacobi_subeig_kernel(const double2 *Kp, i
     const int2 pq = pairs[blockIdx.x];
     const double tiny = norm2[1];
     auto gidx = [&](int a) { return a < EIG_JB ? pq.x * EIG_JB + a : pq.y * EIG_JB + a - EIG_JB; };
-    for (int e = tid; e < D * D; e += 256) {
+    for (int e = tid; e < D * D; e += NT) {
         const int i = e % D, j = e / D;
         const int gi = gidx(i), gj = gidx(j);
         const double2 x = Kp[(int64_t)gj * npad + gi], y = Kp[(int64_t)gi * npad + gj];
@@ -342,55 +350,72 @@ __global__ void __launch_bounds__(256) jacobi_subeig_kernel(const double2 *Kp, i
                 else { i = (step + tid) % (D - 1); j = (step - tid + (D - 1)) % (D - 1); }
                 if (i > j) { const int s = i; i = j; j = s; }
                 const double2 aij = A[i * P + j];
-                const double r = sqrt(aij.x * aij.x + aij.y * aij.y);
+                const double r2 = aij.x * aij.x + aij.y * aij.y;
                 double c = 1.0, s = 0.0, er = 1.0, ei = 0.0;
-                if (r > tiny) {
-                    const double tau = (A[j * P + j].x - A[i * P + i].x) / (2.0 * r);
-                    const double tt = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
-                    c = 1.0 / sqrt(1.0 + tt * tt);
+                if (r2 > tiny * tiny) {
+                    const double ir = rsqrt(r2);                                   // 1 / |a_ij|
+                    const double tau = 0.5 * (A[j * P + j].x - A[i * P + i].x) * ir;
+                    const double q = 1.0 + tau * tau;
+                    const double tt = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + q * rsqrt(q));
+                    c = rsqrt(1.0 + tt * tt);
                     s = tt * c;
-                    er = aij.x / r; ei = -aij.y / r;             // e^{-i phi}
+                    er = aij.x * ir; ei = -aij.y * ir;                             // e^{-i phi}
                     active = 1;
                 }
                 rc[tid] = c; rs[tid] = s; rer[tid] = er; rei[tid] = ei; ri[tid] = i; rj[tid] = j;
             }
             __syncthreads();
-            // columns: A <- A J, V <- V J   (lanes run over rows: pitch 65 is conflict-free)
-            for (int item = tid; item < D * 32; item += 256) {
+            // A <- J^H A J, one 2 x 2 block (rows of pair k1, columns of pair k2) per item; a warp shares k1
+            for (int item = tid; item < 32 * 32; item += NT) {
+                const int k2 = item & 31, k1 = item >> 5;
+                const int i1 = ri[k1], j1 = rj[k1], i2 = ri[k2], j2 = rj[k2];
+                const double c1 = rc[k1], s1 = rs[k1], e1r = rer[k1], e1i = rei[k1];
+                const double c2 = rc[k2], s2 = rs[k2], e2r = rer[k2], e2i = rei[k2];
+                double2 a00 = A[i1 * P + i2], a01 = A[i1 * P + j2], a10 = A[j1 * P + i2], a11 = A[j1 * P + j2];
+                // columns: (x, y) -> (c x - s y e, s x + c y e) with e = e^{-i phi} of pair k2
+                {
+                    const double yr = a01.x * e2r - a01.y * e2i, yi = a01.x * e2i + a01.y * e2r;
+                    const double2 x = a00;
+                    a00 = make_double2(c2 * x.x - s2 * yr, c2 * x.y - s2 * yi);
+                    a01 = make_double2(s2 * x.x + c2 * yr, s2 * x.y + c2 * yi);
+                }
+                {
+                    const double yr = a11.x * e2r - a11.y * e2i, yi = a11.x * e2i + a11.y * e2r;
+                    const double2 x = a10;
+                    a10 = make_double2(c2 * x.x - s2 * yr, c2 * x.y - s2 * yi);
+                    a11 = make_double2(s2 * x.x + c2 * yr, s2 * x.y + c2 * yi);
+                }
+                // rows: (x, y) -> (c x - s y conj(e), s x + c y conj(e)) with e of pair k1
+                {
+                    const double yr = a10.x * e1r + a10.y * e1i, yi = a10.y * e1r - a10.x * e1i;
+                    const double2 x = a00;
+                    a00 = make_double2(c1 * x.x - s1 * yr, c1 * x.y - s1 * yi);
+                    a10 = make_double2(s1 * x.x + c1 * yr, s1 * x.y + c1 * yi);
+                }
+                {
+                    const double yr = a11.x * e1r + a11.y * e1i, yi = a11.y * e1r - a11.x * e1i;
+                    const double2 x = a01;
+                    a01 = make_double2(c1 * x.x - s1 * yr, c1 * x.y - s1 * yi);
+                    a11 = make_double2(s1 * x.x + c1 * yr, s1 * x.y + c1 * yi);
+                }
+                A[i1 * P + i2] = a00; A[i1 * P + j2] = a01; A[j1 * P + i2] = a10; A[j1 * P + j2] = a11;
+            }
+            // V <- V J   (lanes run over rows: pitch 65 is conflict-free)
+            for (int item = tid; item < D * 32; item += NT) {
                 const int row = item % D, k = item / D;
                 const int i = ri[k], j = rj[k];
                 const double c = rc[k], s = rs[k], er = rer[k], ei = rei[k];
-                // J_ii = c, J_ij = s, J_ji = -s e, J_jj = c e   (e = e^{-i phi})
-                {
-                    const double2 x = A[row * P + i], y = A[row * P + j];
-                    const double yer = y.x * er - y.y * ei, yei = y.x * ei + y.y * er;   // y * e
-                    A[row * P + i] = make_double2(c * x.x - s * yer, c * x.y - s * yei);
-                    A[row * P + j] = make_double2(s * x.x + c * yer, s * x.y + c * yei);
-                }
-                {
-                    const double2 x = V[row * P + i], y = V[row * P + j];
-                    const double yer = y.x * er - y.y * ei, yei = y.x * ei + y.y * er;
-                    V[row * P + i] = make_double2(c * x.x - s * yer, c * x.y - s * yei);
-                    V[row * P + j] = make_double2(s * x.x + c * yer, s * x.y + c * yei);
-                }
-            }
-            __syncthreads();
-            // rows: A <- J^H A   (lanes run over columns)
-            for (int item = tid; item < D * 32; item += 256) {
-                const int col = item % D, k = item / D;
-                const int i = ri[k], j = rj[k];
-                const double c = rc[k], s = rs[k], er = rer[k], ei = rei[k];
-                const double2 x = A[i * P + col], y = A[j * P + col];
-                const double ycr = y.x * er + y.y * ei, yci = y.y * er - y.x * ei;       // y * conj(e)
-                A[i * P + col] = make_double2(c * x.x - s * ycr, c * x.y - s * yci);
-                A[j * P + col] = make_double2(s * x.x + c * ycr, s * x.y + c * yci);
+                const double2 x = V[row * P + i], y = V[row * P + j];
+                const double yer = y.x * er - y.y * ei, yei = y.x * ei + y.y * er;
+                V[row * P + i] = make_double2(c * x.x - s * yer, c * x.y - s * yei);
+                V[row * P + j] = make_double2(s * x.x + c * yer, s * x.y + c * yei);
             }
             __syncthreads();
         }
         if (!active) break;
     }
     double2 *J = Jbuf + (int64_t)blockIdx.x * D * D;
-    for (int e = tid; e < D * D; e += 256) {
+    for (int e = tid; e < D * D; e += NT) {
         const int i = e % D, j = e / D;
         J[e] = V[i * P + j];
     }
@@ -402,7 +427,8 @@ __global__ void __launch_bounds__(256) jacobi_subeig_kernel(const double2 *Kp, i
 // transposes (the new K is Hermitian to the last bit off the diagonal blocks); V <- V Jt rides along as one product per
 // (pair, 64-row tile).  Items [0, nk) with nk = npairs (npairs + 1) / 2 are the K blocks (two products, the first
 // result T = K_ab J_b goes back to shared memory as the B operand of the second), items [nk, nk + npairs * tiles)
-// are the V tiles.  8 warps, each 32 rows x 16 columns (4 x 2 DMMA tiles), K = 64; operands K-major with pitch 68.
+// are the V tiles (the driver launches the two ranges on two streams: only the K blocks are on the critical path to the
+// next round's sub-problems).  8 warps, each 32 rows x 16 columns (4 x 2 DMMA tiles), K = 64; operands K-major with pitch 68.
 struct BlockUpdArgs {
     const double2 *Kin;
     double2 *Kout;
@@ -411,6 +437,7 @@ struct BlockUpdArgs {
     int32_t npad, npairs, nk, tiles;
     const int2 *pairs;
     const double2 *Jbuf;
+    int32_t item0;             // first item of this launch (0: K blocks first; nk: the V tiles alone)
 };
 
 __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArgs a)
@@ -424,7 +451,7 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
     const int wm = warp >> 2, wn = warp & 3;
     const int g = lane >> 2, t = lane & 3;
     const int npad = a.npad;
-    const int item = blockIdx.x;
+    const int item = blockIdx.x + a.item0;
     const bool kitem = item < a.nk;
     int ia, ib, r0 = 0;
     if (kitem) {
@@ -457,40 +484,47 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
         cp_async_wait<0>();
         __syncthreads();
     }
-    double cre[4][2][2], cim[4][2][2];
+    // complex products from three real DMMA each (3M, as in gram_kernels.cuh): K1 += a0 b_r, K2 += a_r (b_i - b_r),
+    // K3 += a2 (b_r + b_i) with (a0, a2) = (a_r + a_i, a_i) for a b and (a_r - a_i, -a_i) for conj(a) b; re = K1 - K3, im = K1 + K2
+    double cre[4][2][2], cim[4][2][2], ck3[4][2][2];         // K1, K2, K3; combined into (re, im) in place after each product
     auto zero = [&]() {
 #pragma unroll
         for (int x = 0; x < 4; ++x)
 #pragma unroll
-            for (int y = 0; y < 2; ++y) { cre[x][y][0] = cre[x][y][1] = cim[x][y][0] = cim[x][y][1] = 0.0; }
+            for (int y = 0; y < 2; ++y) { cre[x][y][0] = cre[x][y][1] = cim[x][y][0] = cim[x][y][1] = ck3[x][y][0] = ck3[x][y][1] = 0.0; }
     };
-    // first product: C[m][n] = sum_k S0[m][k] * J_b[k][n]
-    zero();
-    {
-        const double2 *Ap = S0 + (wm * 32 + g) * P + t;
-        const double2 *Bp = S1 + (wn * 16 + g) * P + t;
+    auto product = [&](const double2 *Ap, const double2 *Bp, const bool conj_a) {
+        zero();
 #pragma unroll 4
         for (int kk = 0; kk < D; kk += 4) {
-            double br[2], bi[2];
+            double b0[2], b1[2], b2[2];
 #pragma unroll
-            for (int y = 0; y < 2; ++y) { const double2 v = Bp[y * 8 * P + kk]; br[y] = v.x; bi[y] = v.y; }
+            for (int y = 0; y < 2; ++y) { const double2 v = Bp[y * 8 * P + kk]; b0[y] = v.x; b1[y] = v.y - v.x; b2[y] = v.x + v.y; }
 #pragma unroll
             for (int x = 0; x < 4; ++x) {
                 const double2 v = Ap[x * 8 * P + kk];
-                const double ar = v.x, ai = v.y, nai = -v.y;
+                const double a0 = conj_a ? v.x - v.y : v.x + v.y, a1 = v.x, a2 = conj_a ? -v.y : v.y;
 #pragma unroll
                 for (int y = 0; y < 2; ++y) {
-                    eig_dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
-                    eig_dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
-                }
-#pragma unroll
-                for (int y = 0; y < 2; ++y) {
-                    eig_dmma884(cre[x][y][0], cre[x][y][1], nai, bi[y]);
-                    eig_dmma884(cim[x][y][0], cim[x][y][1], ai, br[y]);
+                    eig_dmma884(cre[x][y][0], cre[x][y][1], a0, b0[y]);
+                    eig_dmma884(cim[x][y][0], cim[x][y][1], a1, b1[y]);
+                    eig_dmma884(ck3[x][y][0], ck3[x][y][1], a2, b2[y]);
                 }
             }
         }
-    }
+#pragma unroll
+        for (int x = 0; x < 4; ++x)
+#pragma unroll
+            for (int y = 0; y < 2; ++y)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const double k1 = cre[x][y][e];
+                    cre[x][y][e] = k1 - ck3[x][y][e];
+                    cim[x][y][e] = k1 + cim[x][y][e];
+                }
+    };
+    // first product: C[m][n] = sum_k S0[m][k] * J_b[k][n]
+    product(S0 + (wm * 32 + g) * P + t, S1 + (wn * 16 + g) * P + t, false);
     if (!kitem) {
 #pragma unroll
         for (int x = 0; x < 4; ++x)
@@ -516,32 +550,7 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
             }
     __syncthreads();
     // second product: C[i][j] = sum_r conj(J_a[r][i]) * T[r][j]
-    zero();
-    {
-        const double2 *Ap = S2 + (wm * 32 + g) * P + t;
-        const double2 *Bp = S0 + (wn * 16 + g) * P + t;
-#pragma unroll 4
-        for (int kk = 0; kk < D; kk += 4) {
-            double br[2], bi[2];
-#pragma unroll
-            for (int y = 0; y < 2; ++y) { const double2 v = Bp[y * 8 * P + kk]; br[y] = v.x; bi[y] = v.y; }
-#pragma unroll
-            for (int x = 0; x < 4; ++x) {
-                const double2 v = Ap[x * 8 * P + kk];
-                const double ar = v.x, ai = v.y, nai = -v.y;
-#pragma unroll
-                for (int y = 0; y < 2; ++y) {
-                    eig_dmma884(cre[x][y][0], cre[x][y][1], ar, br[y]);
-                    eig_dmma884(cim[x][y][0], cim[x][y][1], ar, bi[y]);
-                }
-#pragma unroll
-                for (int y = 0; y < 2; ++y) {
-                    eig_dmma884(cre[x][y][0], cre[x][y][1], ai, bi[y]);
-                    eig_dmma884(cim[x][y][0], cim[x][y][1], nai, br[y]);
-                }
-            }
-        }
-    }
+    product(S2 + (wm * 32 + g) * P + t, S0 + (wn * 16 + g) * P + t, true);
 #pragma unroll
     for (int x = 0; x < 4; ++x)
 #pragma unroll

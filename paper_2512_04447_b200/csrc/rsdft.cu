@@ -150,12 +150,19 @@ struct rsdft_plan {
     int eig_inner = 1;                                // inner sweeps of the 64 x 64 sub-problems per visit
     double eig_stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     cudaEvent_t eg_ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    // block Jacobi runs its critical chain (sub-problems, K update) on a high-priority stream and the V updates on a second one
+    cudaStream_t eg_s_hi = nullptr, eg_s_lo = nullptr;
+    cudaEvent_t eg_sync[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // J ready [2], V update done [2], fork, join
+    int eig_overlap = 1;                              // 0: everything on the caller's stream (lab / comparison)
 
     int64_t last_launches = 0;
 
     ~rsdft_plan()
     {
         for (auto e : eg_ev) if (e) cudaEventDestroy(e);
+        for (auto e : eg_sync) if (e) cudaEventDestroy(e);
+        if (eg_s_hi) cudaStreamDestroy(eg_s_hi);
+        if (eg_s_lo) cudaStreamDestroy(eg_s_lo);
         for (auto e : ev) cudaEventDestroy(e);
         for (int i = 0; i < MAX_STREAMS; ++i) {
             if (s_batch[i]) cudaStreamDestroy(s_batch[i]);
