@@ -178,7 +178,8 @@ int rsdft_subspace_rotate2(rsdft_plan_t *plan, int32_t n, int32_t m, const void 
  * ascending order; C DEVICE n x m column-major (ldc >= n), column j = eigenvector j, normalised C^H S_sub C = I
  * (phases, and bases inside degenerate eigenspaces, are not unique).  1 <= m <= n <= 16384.
  * Runs on `stream` and SYNCHRONISES it with the host (once after the Cholesky for the definiteness check, once
- * per Jacobi sweep for the convergence test); on return the outputs are complete.
+ * per Jacobi sweep for the convergence test); on return the outputs are complete.  The Jacobi rounds run on two
+ * plan-owned streams (a high- and a low-priority one) that start behind `stream` and are joined back into it.
  * Errors: INVALID_ARG, ALLOC, CUDA, NOT_POSITIVE_DEFINITE, NO_CONVERGENCE. */
 int rsdft_subspace_eig(rsdft_plan_t *plan, int32_t n, const void *H_sub, const void *S_sub, int32_t lds,
                        int32_t m, double *lambda, void *C, int32_t ldc, void *stream);

@@ -13,8 +13,9 @@
 //                            blocks (round-robin tournament: nblk-1 rounds visit every pair once = one sweep);
 //                            jacobi_subeig_kernel diagonalises each pair's 64 x 64 Hermitian sub-matrix in shared
 //                            memory (parallel-ordered 2 x 2 rotations) and returns its unitary J; the update
-//                            K <- Jt^H K Jt, V <- V Jt (Jt = all pairs of the round) is ONE launch of DMMA products
-//                            over the 64 x 64 blocks (jacobi_block_update_kernel: J_a^H K_ab J_b per block).
+//                            K <- Jt^H K Jt, V <- V Jt (Jt = all pairs of the round) is DMMA products over the
+//                            64 x 64 blocks (jacobi_block_update_kernel: J_a^H K_ab J_b per block; the driver runs
+//                            the K blocks and the V tiles as two launches on two streams).
 //                            Chosen over Householder tridiagonalisation + QL/D&C because every O(n^3) part is a
 //                            tensor-core product and the method is unconditionally accurate.
 #pragma once
