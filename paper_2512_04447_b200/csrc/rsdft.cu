@@ -939,9 +939,12 @@ int apply_h_impl(rsdft_plan *P, int ncol, const double2 *X, int64_t ldx, double2
 #define RSDFT_GRAM_M3 true
 #define RSDFT_GRAM_MINB 2
 #endif
-#define RSDFT_GRAM_SHAPE RSDFT_GRAM_WGM, RSDFT_GRAM_WGN, RSDFT_GRAM_FA, RSDFT_GRAM_FB, 16, RSDFT_GRAM_STAGES
+#ifndef RSDFT_GRAM_KC       // grid points per pipeline stage
+#define RSDFT_GRAM_KC 16
+#endif
+#define RSDFT_GRAM_SHAPE RSDFT_GRAM_WGM, RSDFT_GRAM_WGN, RSDFT_GRAM_FA, RSDFT_GRAM_FB, RSDFT_GRAM_KC, RSDFT_GRAM_STAGES
 using GCfg = GramCfg<RSDFT_GRAM_SHAPE>;
-constexpr int GRAM_KC = 16;
+constexpr int GRAM_KC = RSDFT_GRAM_KC;
 
 int choose_kslabs(int64_t ntiles, int64_t nchunks, int sms)
 {
