@@ -183,6 +183,8 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
     const size_t smem_sub = (size_t)2 * D * (D + 1) * sizeof(double2);
     const size_t smem_upd = (size_t)3 * D * (D + 4) * sizeof(double2);
     RS_CUDA(cudaFuncSetAttribute(rsdft::jacobi_subeig_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_sub));
+    const size_t smem_cross = (size_t)D * (D + 1) * sizeof(double2);
+    RS_CUDA(cudaFuncSetAttribute(rsdft::jacobi_subeig_cross_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_cross));
     RS_CUDA(cudaFuncSetAttribute(rsdft::jacobi_block_update_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_upd));
     double host[3] = {0.0, 0.0, 0.0};
     RS_CUDA(cudaMemcpyAsync(host, scal, sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -225,7 +227,8 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
             double2 *Jb = P->eg_J.p + (size_t)par * jsz;
             const int2 *pr = P->eg_pairs.p + (size_t)r * npairs;
             if (ovl && gr >= 2) RS_CUDA(cudaStreamWaitEvent(hi, P->eg_sync[2 + par], 0));    // the V update two rounds back has read this J buffer
-            rsdft::jacobi_subeig_kernel<<<npairs, rsdft::EIG_SUB_NT, smem_sub, hi>>>(Kp, npad, pr, Jb, P->eig_inner, scal, r > 0 ? 1 : 0);
+            if (r > 0) rsdft::jacobi_subeig_cross_kernel<<<npairs, 1024, smem_cross, hi>>>(Kp, npad, pr, Jb, P->eig_inner, scal);   // cross pairs
+            else rsdft::jacobi_subeig_kernel<<<npairs, rsdft::EIG_SUB_NT, smem_sub, hi>>>(Kp, npad, pr, Jb, P->eig_inner, scal);     // all pairs
             rsdft::BlockUpdArgs u;
             u.Kin = Kp; u.Kout = Tp; u.Vin = Va; u.Vout = Vb;
             u.npad = npad; u.npairs = npairs; u.nk = npairs * (npairs + 1) / 2; u.tiles = tiles;

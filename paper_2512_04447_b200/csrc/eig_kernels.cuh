@@ -305,10 +305,10 @@ __global__ void __launch_bounds__(256) jacobi_offnorm_kernel(const double2 *Kp, 
 //   tau = (a_jj - a_ii)/(2r), t = sign(tau)/(|tau| + sqrt(1 + tau^2)), c = 1/sqrt(1 + t^2), s = t c,
 //   J = [[c, s], [-s e^{-i phi}, c e^{-i phi}]],   A <- J^H A J.
 // A sweep in which no |a_ij| exceeded `tiny` (passed in norm2[1] = absolute threshold) ends the loop early.
-// cross != 0: only the 32 x 32 index pairs (i in block p, j in block q) are rotated (32 steps of 32 disjoint pairs):
-// over the nblk-1 rounds of a sweep every off-diagonal element is then annihilated exactly once (cyclic Jacobi in
-// a block round-robin ordering); the first round of each sweep runs with cross == 0 and also covers the pairs
-// inside the two diagonal blocks (63 steps).
+// This kernel serves the FIRST round of each sweep: all 63 x 32 index pairs of the 64 x 64 sub-matrix, i.e. also the pairs
+// inside the two diagonal blocks.  The other rounds rotate only the 32 x 32 cross pairs (i in block p, j in block q; 32
+// steps) -- jacobi_subeig_cross_kernel below -- so that over the nblk-1 rounds of a sweep every off-diagonal element is
+// annihilated exactly once (cyclic Jacobi in a block round-robin ordering).
 #ifndef RSDFT_EIG_SUB_NT
 #define RSDFT_EIG_SUB_NT 1024
 #endif
@@ -318,7 +318,7 @@ constexpr int EIG_SUB_NT = RSDFT_EIG_SUB_NT;
 // thread applies them.  A <- J^H A J is done per 2 x 2 block (row pair k1, column pair k2: the column rotation of k2,
 // then the row rotation of k1, on the four elements in registers), so a step needs two barriers and one pass over A.
 __global__ void __launch_bounds__(EIG_SUB_NT) jacobi_subeig_kernel(const double2 *Kp, int npad, const int2 *pairs, double2 *Jbuf,
-                                                                   int inner, const double *norm2, int cross)
+                                                                   int inner, const double *norm2)
 {
     constexpr int D = 2 * EIG_JB, P = D + 1, NT = EIG_SUB_NT;
     extern __shared__ __align__(16) unsigned char eig_smem_raw[];
@@ -342,12 +342,11 @@ __global__ void __launch_bounds__(EIG_SUB_NT) jacobi_subeig_kernel(const double2
     for (int sweep = 0; sweep < inner; ++sweep) {
         if (tid == 0) active = 0;
         __syncthreads();
-        const int nsteps = cross ? EIG_JB : D - 1;
+        const int nsteps = D - 1;
         for (int step = 0; step < nsteps; ++step) {
             if (tid < 32) {
                 int i, j;
-                if (cross) { i = tid; j = EIG_JB + ((tid + step) & (EIG_JB - 1)); }
-                else if (tid == 0) { i = D - 1; j = step; }
+                if (tid == 0) { i = D - 1; j = step; }
                 else { i = (step + tid) % (D - 1); j = (step - tid + (D - 1)) % (D - 1); }
                 if (i > j) { const int s = i; i = j; j = s; }
                 const double2 aij = A[i * P + j];
@@ -419,6 +418,126 @@ __global__ void __launch_bounds__(EIG_SUB_NT) jacobi_subeig_kernel(const double2
     for (int e = tid; e < D * D; e += NT) {
         const int i = e % D, j = e / D;
         J[e] = V[i * P + j];
+    }
+}
+
+// The cross rounds (every round of a sweep but its first) with the sub-matrix and the J accumulator in REGISTERS.  Pair k
+// of step s is (i, j) = (k, 32 + ((k + s) & 31)), so thread (k1 = warp, k2 = lane) of the 1024 owns the 2 x 2 block
+//   rows {k1, 32 + ((k1 + s) & 31)} x columns {k2, 32 + ((k2 + s) & 31)}
+// for the whole kernel: a00 never moves, a01 comes from lane + 1 by a shuffle, a10 / a11 from warp + 1 through a
+// double-buffered shared-memory exchange (64 B per thread and step instead of 256 B of in-place updates: shared-memory
+// bandwidth bounded the in-place version).  The thread on the diagonal (k, k) holds a_ii, a_jj and a_ij of pair k and
+// computes its rotation.  Same arithmetic, in the same order, as jacobi_subeig_kernel with cross != 0.
+__global__ void __launch_bounds__(1024) jacobi_subeig_cross_kernel(const double2 *Kp, int npad, const int2 *pairs, double2 *Jbuf,
+                                                                   int inner, const double *norm2)
+{
+    constexpr int JB = EIG_JB, D = 2 * JB, P = D + 1;
+    extern __shared__ __align__(16) unsigned char eig_smem_raw[];
+    double2 *ex = reinterpret_cast<double2 *>(eig_smem_raw);  // [2 buffers][a10, a11][32][32]; at the end V as [D][P]
+    __shared__ double rc[32], rs[32], rer[32], rei[32];
+    __shared__ double piv_ii[32], piv_jj[32];                  // a_ii, a_jj and a_ij of the coming step's 32 pairs
+    __shared__ double2 piv_ij[32];
+    __shared__ int active;
+    const int tid = threadIdx.x, k2 = tid & 31, k1 = tid >> 5;
+    const int2 pq = pairs[blockIdx.x];
+    const double tiny = norm2[1];
+    auto load = [&](int i, int j) {
+        const int gi = i < JB ? pq.x * JB + i : pq.y * JB + i - JB, gj = j < JB ? pq.x * JB + j : pq.y * JB + j - JB;
+        const double2 x = Kp[(int64_t)gj * npad + gi], y = Kp[(int64_t)gi * npad + gj];
+        return make_double2(0.5 * (x.x + y.x), i == j ? 0.0 : 0.5 * (x.y - y.y));
+    };
+    double2 a00 = load(k1, k2), a01 = load(k1, JB + k2), a10 = load(JB + k1, k2), a11 = load(JB + k1, JB + k2);
+    double2 vx[2], vy[2];                                      // V[row][k2], V[row][32 + ((k2 + s) & 31)] for rows k1, k1 + 32
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+        const int row = k1 + 32 * rr;
+        vx[rr] = make_double2(row == k2 ? 1.0 : 0.0, 0.0);
+        vy[rr] = make_double2(row == JB + k2 ? 1.0 : 0.0, 0.0);
+    }
+    for (int sweep = 0; sweep < inner; ++sweep) {
+        if (tid == 0) active = 0;
+        if (k1 == k2) { piv_ii[k1] = a00.x; piv_jj[k1] = a11.x; piv_ij[k1] = a01; }     // step 0: everything is at home
+        __syncthreads();
+        for (int step = 0; step < JB; ++step) {
+            if (k1 == 0) {                                     // one warp forms the 32 rotations (lane = pair)
+                const double2 aij = piv_ij[k2];
+                const double r2 = aij.x * aij.x + aij.y * aij.y;
+                double c = 1.0, s = 0.0, er = 1.0, ei = 0.0;
+                if (r2 > tiny * tiny) {
+                    const double ir = rsqrt(r2);
+                    const double tau = 0.5 * (piv_jj[k2] - piv_ii[k2]) * ir;
+                    const double q = 1.0 + tau * tau;
+                    const double tt = (tau >= 0.0 ? 1.0 : -1.0) / (fabs(tau) + q * rsqrt(q));
+                    c = rsqrt(1.0 + tt * tt);
+                    s = tt * c;
+                    er = aij.x * ir; ei = -aij.y * ir;
+                    active = 1;
+                }
+                rc[k2] = c; rs[k2] = s; rer[k2] = er; rei[k2] = ei;
+            }
+            __syncthreads();
+            const double c1 = rc[k1], s1 = rs[k1], e1r = rer[k1], e1i = rei[k1];
+            const double c2 = rc[k2], s2 = rs[k2], e2r = rer[k2], e2i = rei[k2];
+            {
+                const double yr = a01.x * e2r - a01.y * e2i, yi = a01.x * e2i + a01.y * e2r;
+                const double2 x = a00;
+                a00 = make_double2(c2 * x.x - s2 * yr, c2 * x.y - s2 * yi);
+                a01 = make_double2(s2 * x.x + c2 * yr, s2 * x.y + c2 * yi);
+            }
+            {
+                const double yr = a11.x * e2r - a11.y * e2i, yi = a11.x * e2i + a11.y * e2r;
+                const double2 x = a10;
+                a10 = make_double2(c2 * x.x - s2 * yr, c2 * x.y - s2 * yi);
+                a11 = make_double2(s2 * x.x + c2 * yr, s2 * x.y + c2 * yi);
+            }
+            {
+                const double yr = a10.x * e1r + a10.y * e1i, yi = a10.y * e1r - a10.x * e1i;
+                const double2 x = a00;
+                a00 = make_double2(c1 * x.x - s1 * yr, c1 * x.y - s1 * yi);
+                a10 = make_double2(s1 * x.x + c1 * yr, s1 * x.y + c1 * yi);
+            }
+            {
+                const double yr = a11.x * e1r + a11.y * e1i, yi = a11.y * e1r - a11.x * e1i;
+                const double2 x = a01;
+                a01 = make_double2(c1 * x.x - s1 * yr, c1 * x.y - s1 * yi);
+                a11 = make_double2(s1 * x.x + c1 * yr, s1 * x.y + c1 * yi);
+            }
+#pragma unroll
+            for (int rr = 0; rr < 2; ++rr) {
+                const double2 x = vx[rr], y = vy[rr];
+                const double yer = y.x * e2r - y.y * e2i, yei = y.x * e2i + y.y * e2r;
+                vx[rr] = make_double2(c2 * x.x - s2 * yer, c2 * x.y - s2 * yei);
+                const double nyx = s2 * x.x + c2 * yer, nyy = s2 * x.y + c2 * yei;
+                vy[rr].x = __shfl_sync(0xffffffffu, nyx, (k2 + 1) & 31);
+                vy[rr].y = __shfl_sync(0xffffffffu, nyy, (k2 + 1) & 31);
+            }
+            // hand the moving elements to the next step's owners
+            double2 *e10 = ex + (((step & 1) * 2 + 0) * 32 + k1) * 32, *e11 = ex + (((step & 1) * 2 + 1) * 32 + k1) * 32;
+            e10[k2] = a10; e11[k2] = a11;
+            // ... and the next step's pivots to warp 0: pair k's a_ij is the a01 of thread (k, k + 1), its a_jj the a11 of (k + 1, k + 1)
+            if (k1 == k2) { piv_ii[k1] = a00.x; piv_jj[(k1 + 31) & 31] = a11.x; }
+            if (k2 == ((k1 + 1) & 31)) piv_ij[k1] = a01;
+            a01.x = __shfl_sync(0xffffffffu, a01.x, (k2 + 1) & 31);
+            a01.y = __shfl_sync(0xffffffffu, a01.y, (k2 + 1) & 31);
+            __syncthreads();
+            const int kn = (k1 + 1) & 31;
+            a10 = ex[(((step & 1) * 2 + 0) * 32 + kn) * 32 + k2];
+            a11 = ex[(((step & 1) * 2 + 1) * 32 + kn) * 32 + ((k2 + 1) & 31)];
+        }
+        if (!active) break;
+    }
+    __syncthreads();                                           // the exchange buffers become the staging area of J
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+        const int row = k1 + 32 * rr;
+        ex[row * P + k2] = vx[rr];
+        ex[row * P + JB + k2] = vy[rr];
+    }
+    __syncthreads();
+    double2 *J = Jbuf + (int64_t)blockIdx.x * D * D;
+    for (int e = tid; e < D * D; e += 1024) {
+        const int i = e % D, j = e / D;
+        J[e] = ex[i * P + j];
     }
 }
 
