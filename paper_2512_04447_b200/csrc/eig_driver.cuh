@@ -255,6 +255,9 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
         RS_CUDA(cudaMemcpyAsync(host + 2, scal + 2, sizeof(double), cudaMemcpyDeviceToHost, hi));
         RS_CUDA(cudaStreamSynchronize(hi));
         const double off = host[2];
+#ifdef RSDFT_LAB_N
+        if (getenv("RSDFT_LAB_EIGTRACE")) fprintf(stderr, "sweep %d: off/norm = %.3e\n", sweep, std::sqrt(off / norm2));
+#endif
         // converged: off(K) <= 1e-13 ||K||_F, or the round-off floor is reached (no further decrease below 1e-10)
         if (off <= 1e-26 * norm2) converged = true;
         else if (prev >= 0.0 && off > 0.25 * prev && off <= 1e-20 * norm2) converged = true;
