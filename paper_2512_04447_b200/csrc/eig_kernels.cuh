@@ -586,23 +586,30 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
     }
     const int2 pa = a.pairs[ia], pb = a.pairs[ib];
     auto idx = [&](int2 pq, int c) { return c < EIG_JB ? pq.x * EIG_JB + c : pq.y * EIG_JB + c - EIG_JB; };
-    // operand loads: S0[m*P + k] = In[row(m) + col_b(k)*npad]; S1 = J_b; S2 = J_a (K items only)
+    // operand loads: S0[m*P + k] = In[row(m) + col_b(k)*npad]; S1 = J_b; S2 = J_a (K items only), as three cp.async groups --
+    // the k < 32 halves of S0 and S1, their k >= 32 halves, S2 -- so that the first product starts on half of its operands
+    // and the loads of the rest hide behind it
     {
         const double2 *In = kitem ? a.Kin : a.Vin;
-        for (int e = tid; e < D * D; e += 256) {
-            const int m = e % D, k = e / D;
-            const int row = kitem ? idx(pa, m) : r0 + m;
-            cp_async16(S0 + m * P + k, In + (int64_t)idx(pb, k) * npad + row);
-        }
         const double2 *Jb = a.Jbuf + (int64_t)ib * D * D;
-        for (int e = tid; e < D * D; e += 256) cp_async16(S1 + (e / D) * P + (e % D), Jb + e);
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            for (int e = tid; e < D * (D / 2); e += 256) {
+                const int m = e % D, k = half * (D / 2) + e / D;
+                const int row = kitem ? idx(pa, m) : r0 + m;
+                cp_async16(S0 + m * P + k, In + (int64_t)idx(pb, k) * npad + row);
+            }
+            for (int e = tid; e < D * (D / 2); e += 256) {
+                const int k = half * (D / 2) + e % (D / 2), n = e / (D / 2);
+                cp_async16(S1 + n * P + k, Jb + n * D + k);
+            }
+            cp_async_commit();
+        }
         if (kitem) {
             const double2 *Ja = a.Jbuf + (int64_t)ia * D * D;
             for (int e = tid; e < D * D; e += 256) cp_async16(S2 + (e / D) * P + (e % D), Ja + e);
         }
         cp_async_commit();
-        cp_async_wait<0>();
-        __syncthreads();
     }
     // complex products from three real DMMA each (3M, as in gram_kernels.cuh): K1 += a0 b_r, K2 += a_r (b_i - b_r),
     // K3 += a2 (b_r + b_i) with (a0, a2) = (a_r + a_i, a_i) for a b and (a_r - a_i, -a_i) for conj(a) b; re = K1 - K3, im = K1 + K2
@@ -613,10 +620,9 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
 #pragma unroll
             for (int y = 0; y < 2; ++y) { cre[x][y][0] = cre[x][y][1] = cim[x][y][0] = cim[x][y][1] = ck3[x][y][0] = ck3[x][y][1] = 0.0; }
     };
-    auto product = [&](const double2 *Ap, const double2 *Bp, const bool conj_a) {
-        zero();
+    auto mac = [&](const double2 *Ap, const double2 *Bp, const bool conj_a, const int k0, const int k1) {
 #pragma unroll 4
-        for (int kk = 0; kk < D; kk += 4) {
+        for (int kk = k0; kk < k1; kk += 4) {
             double b0[2], b1[2], b2[2];
 #pragma unroll
             for (int y = 0; y < 2; ++y) { const double2 v = Bp[y * 8 * P + kk]; b0[y] = v.x; b1[y] = v.y - v.x; b2[y] = v.x + v.y; }
@@ -632,6 +638,8 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
                 }
             }
         }
+    };
+    auto combine = [&]() {
 #pragma unroll
         for (int x = 0; x < 4; ++x)
 #pragma unroll
@@ -643,8 +651,15 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
                     cim[x][y][e] = k1 + cim[x][y][e];
                 }
     };
-    // first product: C[m][n] = sum_k S0[m][k] * J_b[k][n]
-    product(S0 + (wm * 32 + g) * P + t, S1 + (wn * 16 + g) * P + t, false);
+    // first product: C[m][n] = sum_k S0[m][k] * J_b[k][n], the k < 32 half as soon as it has landed
+    zero();
+    cp_async_wait<2>();
+    __syncthreads();
+    mac(S0 + (wm * 32 + g) * P + t, S1 + (wn * 16 + g) * P + t, false, 0, D / 2);
+    cp_async_wait<1>();
+    __syncthreads();
+    mac(S0 + (wm * 32 + g) * P + t, S1 + (wn * 16 + g) * P + t, false, D / 2, D);
+    combine();
     if (!kitem) {
 #pragma unroll
         for (int x = 0; x < 4; ++x)
@@ -668,9 +683,12 @@ __global__ void __launch_bounds__(256, 1) jacobi_block_update_kernel(BlockUpdArg
                 const int m = wm * 32 + x * 8 + g, n = wn * 16 + y * 8 + 2 * t + e;
                 S0[n * P + m] = make_double2(cre[x][y][e], cim[x][y][e]);          // T^T: B operand of the second product
             }
+    cp_async_wait<0>();                                // J_a (S2) has landed
     __syncthreads();
     // second product: C[i][j] = sum_r conj(J_a[r][i]) * T[r][j]
-    product(S2 + (wm * 32 + g) * P + t, S0 + (wn * 16 + g) * P + t, true);
+    zero();
+    mac(S2 + (wm * 32 + g) * P + t, S0 + (wn * 16 + g) * P + t, true, 0, D);
+    combine();
 #pragma unroll
     for (int x = 0; x < 4; ++x)
 #pragma unroll
