@@ -197,24 +197,17 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
     // Two streams per round: `hi` carries the chain sub-problems -> K update -> next sub-problems (the 23 sub-problem
     // CTAs are a latency chain on 23 SMs), `lo` carries V <- V Jt, which nothing needs before the end and which fills
     // the other SMs meanwhile.  J is double-buffered by round parity; ev J[p] = J of that parity written, V[p] = read.
-    bool ovl = P->eig_overlap != 0;
-#ifdef RSDFT_LAB_N
-    if (const char *e = getenv("RSDFT_LAB_EIGOVL")) ovl = atoi(e) != 0;
-#endif
-    cudaStream_t hi = st, lo = st;
-    if (ovl) {
-        if (!P->eg_s_hi) {
-            int plo = 0, phi = 0;
-            RS_CUDA(cudaDeviceGetStreamPriorityRange(&plo, &phi));
-            RS_CUDA(cudaStreamCreateWithPriority(&P->eg_s_hi, cudaStreamNonBlocking, phi));
-            RS_CUDA(cudaStreamCreateWithPriority(&P->eg_s_lo, cudaStreamNonBlocking, plo));
-            for (auto &e : P->eg_sync) RS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-        }
-        hi = P->eg_s_hi; lo = P->eg_s_lo;
-        RS_CUDA(cudaEventRecord(P->eg_sync[4], st));            // fork: both streams start behind the caller's stream
-        RS_CUDA(cudaStreamWaitEvent(hi, P->eg_sync[4], 0));
-        RS_CUDA(cudaStreamWaitEvent(lo, P->eg_sync[4], 0));
+    if (!P->eg_s_hi) {
+        int plo = 0, phi = 0;
+        RS_CUDA(cudaDeviceGetStreamPriorityRange(&plo, &phi));
+        RS_CUDA(cudaStreamCreateWithPriority(&P->eg_s_hi, cudaStreamNonBlocking, phi));
+        RS_CUDA(cudaStreamCreateWithPriority(&P->eg_s_lo, cudaStreamNonBlocking, plo));
+        for (auto &e : P->eg_sync) RS_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     }
+    const cudaStream_t hi = P->eg_s_hi, lo = P->eg_s_lo;
+    RS_CUDA(cudaEventRecord(P->eg_sync[4], st));                // fork: both streams start behind the caller's stream
+    RS_CUDA(cudaStreamWaitEvent(hi, P->eg_sync[4], 0));
+    RS_CUDA(cudaStreamWaitEvent(lo, P->eg_sync[4], 0));
     const size_t jsz = (size_t)npairs * D * D;
     double prev = -1.0;
     int sweep = 0;
@@ -223,28 +216,23 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
     const int max_sweeps = 30;
     for (; sweep < max_sweeps && !converged; ++sweep) {
         for (int r = 0; r < rounds; ++r, ++gr) {
-            const int par = ovl ? (int)(gr & 1) : 0;
+            const int par = (int)(gr & 1);
             double2 *Jb = P->eg_J.p + (size_t)par * jsz;
             const int2 *pr = P->eg_pairs.p + (size_t)r * npairs;
-            if (ovl && gr >= 2) RS_CUDA(cudaStreamWaitEvent(hi, P->eg_sync[2 + par], 0));    // the V update two rounds back has read this J buffer
+            if (gr >= 2) RS_CUDA(cudaStreamWaitEvent(hi, P->eg_sync[2 + par], 0));    // the V update two rounds back has read this J buffer
             if (r > 0) rsdft::jacobi_subeig_cross_kernel<<<npairs, 1024, smem_cross, hi>>>(Kp, npad, pr, Jb, P->eig_inner, scal);   // cross pairs
             else rsdft::jacobi_subeig_kernel<<<npairs, rsdft::EIG_SUB_NT, smem_sub, hi>>>(Kp, npad, pr, Jb, P->eig_inner, scal);     // all pairs
             rsdft::BlockUpdArgs u;
             u.Kin = Kp; u.Kout = Tp; u.Vin = Va; u.Vout = Vb;
             u.npad = npad; u.npairs = npairs; u.nk = npairs * (npairs + 1) / 2; u.tiles = tiles;
             u.pairs = pr; u.Jbuf = Jb; u.item0 = 0;
-            if (ovl) {
-                RS_CUDA(cudaEventRecord(P->eg_sync[par], hi));
-                rsdft::jacobi_block_update_kernel<<<u.nk, 256, smem_upd, hi>>>(u);                       // K = Jt^H K Jt
-                RS_CUDA(cudaStreamWaitEvent(lo, P->eg_sync[par], 0));
-                u.item0 = u.nk;
-                rsdft::jacobi_block_update_kernel<<<npairs * tiles, 256, smem_upd, lo>>>(u);             // V = V Jt
-                RS_CUDA(cudaEventRecord(P->eg_sync[2 + par], lo));
-                P->last_launches += 3;
-            } else {
-                rsdft::jacobi_block_update_kernel<<<u.nk + npairs * tiles, 256, smem_upd, st>>>(u);      // both in one launch
-                P->last_launches += 2;
-            }
+            RS_CUDA(cudaEventRecord(P->eg_sync[par], hi));
+            rsdft::jacobi_block_update_kernel<<<u.nk, 256, smem_upd, hi>>>(u);                           // K = Jt^H K Jt
+            RS_CUDA(cudaStreamWaitEvent(lo, P->eg_sync[par], 0));
+            u.item0 = u.nk;
+            rsdft::jacobi_block_update_kernel<<<npairs * tiles, 256, smem_upd, lo>>>(u);                 // V = V Jt
+            RS_CUDA(cudaEventRecord(P->eg_sync[2 + par], lo));
+            P->last_launches += 3;
             std::swap(Kp, Tp);
             std::swap(Va, Vb);
         }
@@ -263,12 +251,10 @@ static int eig_jacobi(rsdft_plan *P, int n, int m, int lower_only, double *lambd
         else if (prev >= 0.0 && off > 0.25 * prev && off <= 1e-20 * norm2) converged = true;
         prev = off;
     }
-    if (ovl) {                                                  // join: the caller's stream continues behind both
-        RS_CUDA(cudaEventRecord(P->eg_sync[5], lo));
-        RS_CUDA(cudaStreamWaitEvent(st, P->eg_sync[5], 0));
-        RS_CUDA(cudaEventRecord(P->eg_sync[5], hi));
-        RS_CUDA(cudaStreamWaitEvent(st, P->eg_sync[5], 0));
-    }
+    RS_CUDA(cudaEventRecord(P->eg_sync[5], lo));                // join: the caller's stream continues behind both
+    RS_CUDA(cudaStreamWaitEvent(st, P->eg_sync[5], 0));
+    RS_CUDA(cudaEventRecord(P->eg_sync[5], hi));
+    RS_CUDA(cudaStreamWaitEvent(st, P->eg_sync[5], 0));
     P->eig_stats[0] = sweep;
     P->eig_stats[5] = norm2 > 0.0 ? std::sqrt(prev < 0.0 ? 0.0 : prev / norm2) : 0.0;
     if (!converged) return fail(RSDFT_NO_CONVERGENCE, "rsdft_subspace_eig: block Jacobi did not converge in 30 sweeps");

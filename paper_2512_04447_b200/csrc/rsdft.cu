@@ -153,7 +153,6 @@ struct rsdft_plan {
     // block Jacobi runs its critical chain (sub-problems, K update) on a high-priority stream and the V updates on a second one
     cudaStream_t eg_s_hi = nullptr, eg_s_lo = nullptr;
     cudaEvent_t eg_sync[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // J ready [2], V update done [2], fork, join
-    int eig_overlap = 1;                              // 0: everything on the caller's stream (lab / comparison)
 
     int64_t last_launches = 0;
 
