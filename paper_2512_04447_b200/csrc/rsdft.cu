@@ -134,7 +134,7 @@ struct rsdft_plan {
 
     // host-buffer entry point
     DevBuf<double2> hostY, hostHY, hostHS;
-    cudaStream_t s_copy = nullptr, s_comp = nullptr;
+    cudaStream_t s_copy = nullptr, s_comp = nullptr, s_h = nullptr;
     std::vector<cudaEvent_t> ev;
     cudaEvent_t ev_vloc = nullptr;                    // recorded by set_vloc on the caller's stream; block_step_host waits on it
     bool vloc_pending = false;
@@ -171,6 +171,7 @@ struct rsdft_plan {
         if (ev_vloc) cudaEventDestroy(ev_vloc);
         if (s_copy) cudaStreamDestroy(s_copy);
         if (s_comp) cudaStreamDestroy(s_comp);
+        if (s_h) cudaStreamDestroy(s_h);
     }
     size_t device_bytes() const
     {
@@ -1386,13 +1387,20 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     RS_CUDA(P->hostHS.ensure((size_t)2 * n * n));
     if (!P->s_copy) RS_CUDA(cudaStreamCreateWithFlags(&P->s_copy, cudaStreamNonBlocking));
     if (!P->s_comp) RS_CUDA(cudaStreamCreateWithFlags(&P->s_comp, cudaStreamNonBlocking));
+    if (!P->s_h) {
+        int plo = 0, phi = 0;
+        RS_CUDA(cudaDeviceGetStreamPriorityRange(&plo, &phi));
+        RS_CUDA(cudaStreamCreateWithPriority(&P->s_h, cudaStreamNonBlocking, phi));
+    }
+    const cudaStream_t sh = P->s_h;     // apply_h on its own high-priority stream: panel k+1 goes through H in the tail of panel k's Gram launch
     // a V_loc set on some caller stream must have landed before the plan-owned streams read it
     if (P->vloc_pending) {
         RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev_vloc, 0));
+        RS_CUDA(cudaStreamWaitEvent(P->s_h, P->ev_vloc, 0));
         P->vloc_pending = false;
     }
-    // Column panels of two Gram tile widths (96 columns; apply_h keeps efficient batches): the H2D copy of panel k+1 overlaps apply_h and
-    // the Gram tiles of panel k.  After panel t has been through H, every [S|H] tile that involves only
+    // Column panels of two Gram tile widths (96 columns; apply_h keeps efficient batches) on three plan-owned streams (copy, H, Gram): the
+    // H2D copy of panel k+1 overlaps apply_h and the Gram tiles of panel k, and apply_h of panel k+1 fills the tail of panel k's Gram launch.  After panel t has been through H, every [S|H] tile that involves only
     // columns < TM(t+1) and touches panel t is contracted, so the Gram (the long part of the step) runs
     // while the rest of Y is still crossing PCIe instead of after the last byte has arrived.
     constexpr int TPP = 2;                                     // Gram tile columns per upload panel
@@ -1434,12 +1442,13 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
 #ifdef RSDFT_LAB_TIMELINE
             cudaEventRecord(tl[3 * k], P->s_copy);
 #endif
-            RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev[2 * k], 0));
-            int r = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, P->s_comp);
+            RS_CUDA(cudaStreamWaitEvent(sh, P->ev[2 * k], 0));
+            int r = apply_h_impl(P, nc, P->hostY.p + (int64_t)c0 * ng, ng, P->hostHY.p + (int64_t)c0 * ng, ng, sh);
             if (r != RSDFT_OK) return r;
-            RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], P->s_comp));
+            RS_CUDA(cudaEventRecord(P->ev[2 * k + 1], sh));
+            RS_CUDA(cudaStreamWaitEvent(P->s_comp, P->ev[2 * k + 1], 0));
 #ifdef RSDFT_LAB_TIMELINE
-            cudaEventRecord(tl[3 * k + 1], P->s_comp);
+            cudaEventRecord(tl[3 * k + 1], sh);
 #endif
             launches += P->last_launches;
             P->last_launches = 0;
@@ -1468,7 +1477,7 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
         return RSDFT_OK;
     };
     rc = body();
-    const cudaError_t e1 = cudaStreamSynchronize(P->s_comp), e2 = cudaStreamSynchronize(P->s_copy);
+    const cudaError_t e0 = cudaStreamSynchronize(P->s_h), e1 = cudaStreamSynchronize(P->s_comp), e2 = cudaStreamSynchronize(P->s_copy);
 #ifdef RSDFT_LAB_TIMELINE
     for (int k = 0; k < nchunk; ++k) {
         float t[3];
@@ -1479,6 +1488,7 @@ int rsdft_block_step_host(rsdft_plan_t *plan, int32_t n, const void *Y_host, int
     for (auto &e : tl) cudaEventDestroy(e);
 #endif
     if (rc != RSDFT_OK) return rc;
+    RS_CUDA(e0);
     RS_CUDA(e1);
     RS_CUDA(e2);
     return RSDFT_OK;
